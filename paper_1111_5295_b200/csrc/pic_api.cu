@@ -1,0 +1,301 @@
+// pic_api.cu — the C-ABI of include/pic.h: handle life cycle, binning, move, residual, commit,
+// getters.  Argument marshalling and launches only; the arithmetic of the path is in mover.cuh.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "mover.cuh"
+#include "pic_internal.h"
+#include "pic_kernels.cuh"
+
+namespace picb200 {
+
+int set_err(pic_handle* h, int code, const char* what, cudaError_t ce) {
+  if (h) {
+    h->err = what ? what : "";
+    if (ce != cudaSuccess) {
+      h->err += ": ";
+      h->err += cudaGetErrorString(ce);
+    }
+  }
+  return code;
+}
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+namespace {
+
+int grid_for(long long n, int threads = 256, int cap = 148 * 16) {
+  long long g = (n + threads - 1) / threads;
+  return (int)std::max<long long>(1, std::min<long long>(g, cap));
+}
+
+// Bring a caller grid array to the device (no-op for device pointers).
+int to_device(pic_handle* h, const double* src, double* staging, const double** out) {
+  if (is_device_ptr(src)) { *out = src; return PIC_OK; }
+  PIC_CUDA(h, cudaMemcpyAsync(staging, src, sizeof(double) * h->grid.n_cells,
+                              cudaMemcpyHostToDevice, h->stream));
+  *out = staging;
+  return PIC_OK;
+}
+
+// Deliver a device grid array to the caller (host: copy + synchronise).
+int from_device(pic_handle* h, const double* dsrc, double* dst) {
+  if (!dst) return PIC_OK;
+  const bool dev = is_device_ptr(dst);
+  PIC_CUDA(h, cudaMemcpyAsync(dst, dsrc, sizeof(double) * h->grid.n_cells,
+                              dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+  if (!dev) PIC_CUDA(h, cudaStreamSynchronize(h->stream));
+  return PIC_OK;
+}
+
+template <typename T>
+int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double* dv_) {
+  const int32_t ng = h->grid.n_cells;
+  const double dx = h->grid.length / ng;
+  const int b = h->cur;
+  // stage 1: cell/xi/v in input order into buffer 1-b, histogram
+  PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (ng + 1), h->stream));
+  bin_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, dx_, dv_, dx, h->grid.length, ng,
+                                                      S.cell[1 - b], (T*)S.xi[1 - b],
+                                                      (T*)S.v[1 - b], h->d_hist, h->d_flag);
+  scan_kernel<<<1, 1024, 0, h->stream>>>(ng, h->d_hist);
+  scatter_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(
+      S.n, S.cell[1 - b], (const T*)S.xi[1 - b], (const T*)S.v[1 - b], nullptr, h->d_hist,
+      S.cell[b], (T*)S.xi[b], (T*)S.v[b], S.id[b]);
+  h->launches += 3;
+  PIC_CUDA(h, cudaGetLastError());
+  return PIC_OK;
+}
+
+template <typename T>
+int rebin_species(pic_handle* h, SpeciesState& S) {
+  // state n+1 lives in buffer 1-cur; scatter it, binned, into buffer cur (old state n is dead).
+  const int32_t ng = h->grid.n_cells;
+  const int src = 1 - h->cur, dst = h->cur;
+  PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (ng + 1), h->stream));
+  hist_kernel<<<grid_for(S.n), 256, 0, h->stream>>>(S.n, S.cell[src], h->d_hist);
+  scan_kernel<<<1, 1024, 0, h->stream>>>(ng, h->d_hist);
+  // ids: buffer 1-cur was written in the order of buffer cur, so its ids are id[cur]; the
+  // re-binned ids go to id[1-cur] and the two id arrays then trade places.
+  scatter_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(
+      S.n, S.cell[src], (const T*)S.xi[src], (const T*)S.v[src], S.id[dst], h->d_hist,
+      S.cell[dst], (T*)S.xi[dst], (T*)S.v[dst], S.id[src]);
+  std::swap(S.id[0], S.id[1]);
+  h->launches += 3;
+  PIC_CUDA(h, cudaGetLastError());
+  return PIC_OK;
+}
+
+void free_all(pic_handle* h) {
+  for (auto& S : h->sp) {
+    for (int b = 0; b < 2; ++b) {
+      cudaFree(S.xi[b]); cudaFree(S.v[b]); cudaFree(S.cell[b]); cudaFree(S.id[b]);
+    }
+    cudaFree(S.nsub); cudaFree(S.ncross);
+  }
+  cudaFree(h->dE_n); cudaFree(h->dE_step); cudaFree(h->dE_np1); cudaFree(h->d_jbar);
+  cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue); cudaFree(h->d_stats);
+  cudaFree(h->d_hist); cudaFree(h->d_flag);
+  if (h->ev0) cudaEventDestroy(h->ev0);
+  if (h->ev1) cudaEventDestroy(h->ev1);
+}
+
+thread_local std::string g_init_err;
+
+}  // namespace
+}  // namespace picb200
+
+using namespace picb200;
+
+extern "C" {
+
+int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species, int n_species,
+             const double* const* x, const double* const* v, const pic_params* params,
+             void* stream) {
+  if (!out) return PIC_ERR_ARG;
+  *out = nullptr;
+  if (!grid || !species || !x || !v || !params || n_species < 1 || grid->n_cells < 1 ||
+      !(grid->length > 0.0) || !(params->eps_a > 0.0) || !(params->eps_r > 0.0) ||
+      !(params->kappa_max > 0.0 && params->kappa_max < 1.0) || params->max_substeps < 1 ||
+      (params->precision != PIC_FP32 && params->precision != PIC_FP64) ||
+      (params->cn_mode != PIC_CN_PICARD && params->cn_mode != PIC_CN_DIRECT))
+    return PIC_ERR_ARG;
+  for (int s = 0; s < n_species; ++s)
+    if (species[s].n < 0 || species[s].n > 0xffffffffLL || !x[s] || !v[s] ||
+        species[s].q_over_m == 0.0)
+      return PIC_ERR_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return PIC_ERR_CUDA;   // no CPU fallback
+  }
+  pic_handle* h = new (std::nothrow) pic_handle();
+  if (!h) return PIC_ERR_ARG;
+  h->grid = *grid;
+  h->params = *params;
+  if (h->params.picard_max < 1) h->params.picard_max = 100;
+  h->stream = (cudaStream_t)stream;
+  h->elem = params->precision == PIC_FP32 ? 4 : 8;
+  int rc = PIC_OK;
+  auto fail = [&](int code) { free_all(h); g_init_err = h->err; delete h; return code; };
+  {
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+      return fail(set_err(h, PIC_ERR_CUDA, "cudaGetDeviceProperties"));
+    h->sm_count = prop.multiProcessorCount;
+  }
+  const int32_t ng = grid->n_cells;
+#define INIT_CUDA(call)                                                                    \
+  do {                                                                                     \
+    cudaError_t ce_ = (call);                                                              \
+    if (ce_ != cudaSuccess) return fail(set_err(h, PIC_ERR_CUDA, #call, ce_));             \
+  } while (0)
+  INIT_CUDA(cudaMalloc(&h->dE_n, sizeof(double) * ng));
+  INIT_CUDA(cudaMalloc(&h->dE_step, sizeof(double) * ng));
+  INIT_CUDA(cudaMalloc(&h->dE_np1, sizeof(double) * ng));
+  INIT_CUDA(cudaMalloc(&h->d_jbar, sizeof(double) * ng));
+  INIT_CUDA(cudaMalloc(&h->d_resid, sizeof(double) * ng));
+  INIT_CUDA(cudaMalloc(&h->d_queue, sizeof(unsigned long long) * n_species));
+  INIT_CUDA(cudaMalloc(&h->d_stats, sizeof(unsigned long long) * ST_COUNT));
+  INIT_CUDA(cudaMalloc(&h->d_hist, sizeof(int32_t) * (ng + 1)));
+  INIT_CUDA(cudaMalloc(&h->d_flag, sizeof(int32_t)));
+  INIT_CUDA(cudaMemsetAsync(h->d_flag, 0, sizeof(int32_t), h->stream));
+  INIT_CUDA(cudaEventCreate(&h->ev0));
+  INIT_CUDA(cudaEventCreate(&h->ev1));
+  h->sp.resize(n_species);
+  for (int s = 0; s < n_species; ++s) {
+    SpeciesState& S = h->sp[s];
+    S.n = species[s].n;
+    S.q_over_m = species[s].q_over_m;
+    S.w_q = species[s].macro_charge;
+    const size_t n1 = (size_t)std::max<long long>(S.n, 1);
+    for (int b = 0; b < 2; ++b) {
+      INIT_CUDA(cudaMalloc(&S.xi[b], h->elem * n1));
+      INIT_CUDA(cudaMalloc(&S.v[b], h->elem * n1));
+      INIT_CUDA(cudaMalloc(&S.cell[b], sizeof(int32_t) * n1));
+      INIT_CUDA(cudaMalloc(&S.id[b], sizeof(uint32_t) * n1));
+    }
+    if (params->flags & PIC_FLAG_COUNTS) {
+      INIT_CUDA(cudaMalloc(&S.nsub, sizeof(uint32_t) * n1));
+      INIT_CUDA(cudaMalloc(&S.ncross, sizeof(uint32_t) * n1));
+    }
+    if (S.n == 0) continue;
+    // inputs: device pointers are used in place, host arrays go through a temporary
+    const double* dxp = x[s];
+    const double* dvp = v[s];
+    double *tx = nullptr, *tv = nullptr;
+    if (!is_device_ptr(x[s])) {
+      INIT_CUDA(cudaMalloc(&tx, sizeof(double) * S.n));
+      INIT_CUDA(cudaMemcpyAsync(tx, x[s], sizeof(double) * S.n, cudaMemcpyHostToDevice, h->stream));
+      dxp = tx;
+    }
+    if (!is_device_ptr(v[s])) {
+      cudaError_t e = cudaMalloc(&tv, sizeof(double) * S.n);
+      if (e == cudaSuccess)
+        e = cudaMemcpyAsync(tv, v[s], sizeof(double) * S.n, cudaMemcpyHostToDevice, h->stream);
+      if (e != cudaSuccess) { cudaFree(tx); cudaFree(tv); return fail(set_err(h, PIC_ERR_CUDA, "upload v", e)); }
+      dvp = tv;
+    }
+    rc = h->elem == 4 ? bin_species<float>(h, S, dxp, dvp) : bin_species<double>(h, S, dxp, dvp);
+    cudaStreamSynchronize(h->stream);
+    cudaFree(tx);
+    cudaFree(tv);
+    if (rc != PIC_OK) return fail(rc);
+  }
+  int32_t flag = 0;
+  INIT_CUDA(cudaMemcpyAsync(&flag, h->d_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream));
+  INIT_CUDA(cudaStreamSynchronize(h->stream));
+  if (flag) return fail(set_err(h, PIC_ERR_PARTICLE, "particle with x outside [0,L) or non-finite x/v"));
+  rc = mover_configure(h);
+  if (rc != PIC_OK) return fail(rc);
+  INIT_CUDA(cudaMalloc(&h->d_partial, sizeof(double) * (size_t)std::max(h->total_rows, 1) * ng));
+#undef INIT_CUDA
+  *out = h;
+  return PIC_OK;
+}
+
+int pic_move_accumulate(pic_handle* h, const double* E_n, const double* E_np1, double dt,
+                        double tol, double* jbar_out) {
+  if (!h) return PIC_ERR_ARG;
+  if (!E_n || !E_np1 || !(dt > 0.0) || !(tol >= 0.0)) return set_err(h, PIC_ERR_ARG, "pic_move_accumulate: bad argument");
+  const double *dEn = nullptr, *dEp = nullptr;
+  int rc;
+  if ((rc = to_device(h, E_n, h->dE_n, &dEn)) != PIC_OK) return rc;
+  if ((rc = to_device(h, E_np1, h->dE_np1, &dEp)) != PIC_OK) return rc;
+  const int ns = (int)h->sp.size();
+  PIC_CUDA(h, cudaMemsetAsync(h->d_queue, 0, sizeof(unsigned long long) * ns, h->stream));
+  PIC_CUDA(h, cudaMemsetAsync(h->d_stats, 0, sizeof(unsigned long long) * ST_COUNT, h->stream));
+  PIC_CUDA(h, cudaEventRecord(h->ev0, h->stream));
+  int row = 0;
+  for (int s = 0; s < ns; ++s) {
+    if ((rc = launch_mover(h, s, dEn, dEp, dt, tol, row)) != PIC_OK) return rc;
+    row += h->sp[s].grid_blocks;
+  }
+  PIC_CUDA(h, cudaEventRecord(h->ev1, h->stream));
+  const int32_t ng = h->grid.n_cells;
+  reduce_rows_kernel<<<(ng + 127) / 128, 128, 0, h->stream>>>(row, ng, h->d_partial, h->d_jbar);
+  h->launches++;
+  PIC_CUDA(h, cudaGetLastError());
+  h->have_np1 = !(h->params.flags & PIC_FLAG_NO_STORE);
+  const bool host_out = jbar_out && !is_device_ptr(jbar_out);
+  unsigned long long capped = 0;
+  if (host_out)   // rides on the synchronisation the host copy of jbar needs anyway
+    PIC_CUDA(h, cudaMemcpyAsync(&capped, h->d_stats + ST_SUBSTEP_CAP, sizeof capped,
+                                cudaMemcpyDeviceToHost, h->stream));
+  if ((rc = from_device(h, h->d_jbar, jbar_out)) != PIC_OK) return rc;
+  if (capped) return set_err(h, PIC_ERR_SUBSTEP_CAP, "particles cut off at max_substeps");
+  return PIC_OK;
+}
+
+int pic_set_step(pic_handle* h, const double* E_n, double dt, double tol) {
+  if (!h) return PIC_ERR_ARG;
+  if (!E_n || !(dt > 0.0) || !(tol >= 0.0)) return set_err(h, PIC_ERR_ARG, "pic_set_step: bad argument");
+  PIC_CUDA(h, cudaMemcpyAsync(h->dE_step, E_n, sizeof(double) * h->grid.n_cells,
+                              is_device_ptr(E_n) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
+                              h->stream));
+  h->step_dt = dt;
+  h->step_tol = tol;
+  h->have_step = true;
+  return PIC_OK;
+}
+
+int pic_residual(pic_handle* h, const double* E_np1, double* resid_out) {
+  if (!h) return PIC_ERR_ARG;
+  if (!h->have_step) return set_err(h, PIC_ERR_STATE, "pic_residual before pic_set_step");
+  if (!E_np1 || !resid_out) return set_err(h, PIC_ERR_ARG, "pic_residual: NULL argument");
+  const double* dEp = nullptr;
+  int rc;
+  if ((rc = to_device(h, E_np1, h->dE_np1, &dEp)) != PIC_OK) return rc;
+  if ((rc = pic_move_accumulate(h, h->dE_step, dEp, h->step_dt, h->step_tol, nullptr)) != PIC_OK)
+    return rc;
+  residual_kernel<<<1, 256, 0, h->stream>>>(h->grid.n_cells, h->dE_step, dEp, h->step_dt,
+                                            h->d_jbar, h->d_resid);
+  h->launches++;
+  PIC_CUDA(h, cudaGetLastError());
+  return from_device(h, h->d_resid, resid_out);
+}
+
+int pic_commit(pic_handle* h) {
+  if (!h) return PIC_ERR_ARG;
+  if (!h->have_np1) return set_err(h, PIC_ERR_STATE, "pic_commit without a stored state n+1");
+  for (auto& S : h->sp) {
+    if (S.n == 0) continue;
+    int rc = h->elem == 4 ? rebin_species<float>(h, S) : rebin_species<double>(h, S);
+    if (rc != PIC_OK) return rc;
+  }
+  h->have_np1 = false;
+  return PIC_OK;
+}
+
+}  // extern "C"

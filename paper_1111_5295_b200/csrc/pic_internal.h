@@ -1,0 +1,75 @@
+// pic_internal.h — handle layout and host-side helpers of the C-ABI library (not exported).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/pic.h"
+
+namespace picb200 {
+
+// One species' device state.  Two SoA buffers (state n / n+1), binned by cell.
+struct SpeciesState {
+  long long n = 0;
+  double q_over_m = 0, w_q = 0;
+  void* xi[2] = {nullptr, nullptr};       // T[n] in-cell offset, cell units
+  void* v[2] = {nullptr, nullptr};        // T[n]
+  int32_t* cell[2] = {nullptr, nullptr};  // int32[n]
+  uint32_t* id[2] = {nullptr, nullptr};   // original index of the particle in each slot
+  uint32_t* nsub = nullptr;               // optional per-particle counts of the last move
+  uint32_t* ncross = nullptr;
+  int grid_blocks = 0;                    // mover launch shape for this species
+  int tile = 0;
+};
+
+}  // namespace picb200
+
+struct pic_handle {
+  pic_grid grid{};
+  pic_params params{};
+  std::vector<picb200::SpeciesState> sp;
+  cudaStream_t stream = nullptr;
+  int cur = 0;                 // index of the buffer holding state n
+  bool have_np1 = false;       // a move has produced state n+1 since the last commit
+  bool have_step = false;      // pic_set_step was called
+  double step_dt = 0, step_tol = 0;
+  size_t elem = 4;             // sizeof(T)
+  int sm_count = 0;
+  int blocks_per_sm = 2;
+  size_t smem_bytes = 0;
+  // device scratch
+  double* dE_n = nullptr;      // [n_cells] staging for host E^n / stored E^n of pic_set_step
+  double* dE_step = nullptr;   // [n_cells] E^n of pic_set_step
+  double* dE_np1 = nullptr;
+  double* d_jbar = nullptr;
+  double* d_resid = nullptr;
+  double* d_partial = nullptr; // [total_rows][n_cells]
+  int total_rows = 0;
+  unsigned long long* d_queue = nullptr;  // [n_species]
+  unsigned long long* d_stats = nullptr;  // [ST_COUNT]
+  int32_t* d_hist = nullptr;              // [n_cells + 1] binning scratch
+  int32_t* d_flag = nullptr;              // validation flag
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  pic_stats stats{};
+  long long launches = 0;
+  std::string err;
+};
+
+namespace picb200 {
+
+int set_err(pic_handle* h, int code, const char* what, cudaError_t ce = cudaSuccess);
+bool is_device_ptr(const void* p);
+// mover launch (pic_mover.cu)
+int launch_mover(pic_handle* h, int s, const double* dE_n, const double* dE_np1, double dt,
+                 double tol, int row0);
+int mover_configure(pic_handle* h);
+
+}  // namespace picb200
+
+#define PIC_CUDA(h, call)                                                        \
+  do {                                                                           \
+    cudaError_t ce_ = (call);                                                    \
+    if (ce_ != cudaSuccess) return picb200::set_err((h), PIC_ERR_CUDA, #call, ce_); \
+  } while (0)

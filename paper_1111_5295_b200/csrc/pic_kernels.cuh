@@ -1,0 +1,191 @@
+// pic_kernels.cuh — small device kernels around the mover: binning by cell,
+// block-partial reduction (a8), Ampere residual (a9), diagnostics.  None of these is the hot loop.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace picb200 {
+
+// x -> (cell, xi): cell = floor(x/dx) clipped to [0, n_cells-1], xi = x/dx - cell clipped to
+// [0,1] and rounded to T.  Also the per-cell histogram and input validation (flag != 0 if any
+// x is outside [0,L) or x / v is not finite).
+template <typename T>
+__global__ void bin_kernel(long long n, const double* __restrict__ x, const double* __restrict__ v,
+                           double dx, double length, int32_t n_cells, int32_t* __restrict__ cell,
+                           T* __restrict__ xi, T* __restrict__ vout, int32_t* __restrict__ hist,
+                           int32_t* __restrict__ flag) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const double xv = x[i], vv = v[i];
+    if (!(xv >= 0.0 && xv < length) || !isfinite(vv)) { atomicOr(flag, 1); }
+    const double u = xv / dx;
+    double fc = floor(u);
+    if (!(fc >= 0.0)) fc = 0.0;
+    if (fc > (double)(n_cells - 1)) fc = (double)(n_cells - 1);
+    const int32_t c = (int32_t)fc;
+    double o = u - fc;
+    o = o < 0.0 ? 0.0 : (o > 1.0 ? 1.0 : o);
+    cell[i] = c;
+    xi[i] = (T)o;
+    vout[i] = (T)vv;
+    atomicAdd(&hist[c], 1);
+  }
+}
+
+static __global__ void hist_kernel(long long n, const int32_t* __restrict__ cell, int32_t* __restrict__ hist) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x)
+    atomicAdd(&hist[cell[i]], 1);
+}
+
+// Exclusive scan of hist[0..n_cells) in place (one block; n_cells is a few thousand at most).
+static __global__ void scan_kernel(int32_t n_cells, int32_t* __restrict__ hist) {
+  __shared__ int32_t carry;
+  __shared__ int32_t wsum[32];
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int base = 0; base < n_cells; base += blockDim.x) {
+    const int i = base + threadIdx.x;
+    const int32_t val = i < n_cells ? hist[i] : 0;
+    int32_t inc = val;
+    for (int o = 1; o < 32; o <<= 1) {
+      const int32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+      int32_t s = lane < (int)(blockDim.x >> 5) ? wsum[lane] : 0;
+      for (int o = 1; o < 32; o <<= 1) {
+        const int32_t t = __shfl_up_sync(0xffffffffu, s, o);
+        if (lane >= o) s += t;
+      }
+      wsum[lane] = s;   // inclusive over warps
+    }
+    __syncthreads();
+    const int32_t woff = w ? wsum[w - 1] : 0;
+    if (i < n_cells) hist[i] = carry + woff + inc - val;
+    __syncthreads();
+    if (threadIdx.x == 0) carry += wsum[(blockDim.x >> 5) - 1];
+    __syncthreads();
+  }
+}
+
+// Scatter into cell bins.  hist holds the running cursor of each cell (exclusive scan at entry).
+// Order inside a bin is arbitrary; `id` carries the original index.
+template <typename T>
+__global__ void scatter_kernel(long long n, const int32_t* __restrict__ cell_in,
+                               const T* __restrict__ xi_in, const T* __restrict__ v_in,
+                               const uint32_t* __restrict__ id_in, int32_t* __restrict__ cursor,
+                               int32_t* __restrict__ cell_out, T* __restrict__ xi_out,
+                               T* __restrict__ v_out, uint32_t* __restrict__ id_out) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const int32_t c = cell_in[i];
+    const int32_t dst = atomicAdd(&cursor[c], 1);
+    cell_out[dst] = c;
+    xi_out[dst] = xi_in[i];
+    v_out[dst] = v_in[i];
+    id_out[dst] = id_in ? id_in[i] : (uint32_t)i;
+  }
+}
+
+// a8: jbar_f = sum over block rows (fixed order -> reproducible given the rows).
+static __global__ void reduce_rows_kernel(int rows, int32_t n_cells, const double* __restrict__ partial,
+                                   double* __restrict__ jbar) {
+  const int f = blockIdx.x * blockDim.x + threadIdx.x;
+  if (f >= n_cells) return;
+  double s = 0.0;
+  for (int r = 0; r < rows; ++r) s += partial[(size_t)r * n_cells + f];
+  jbar[f] = s;
+}
+
+// a9: R_f = (E^{n+1}_f - E^n_f)/dt + jbar_f - <jbar>  (eps0 = 1).  One block.
+static __global__ void residual_kernel(int32_t n_cells, const double* __restrict__ E_n,
+                                const double* __restrict__ E_np1, double dt,
+                                const double* __restrict__ jbar, double* __restrict__ resid) {
+  __shared__ double red[32];
+  __shared__ double mean;
+  double s = 0.0;
+  for (int f = threadIdx.x; f < n_cells; f += blockDim.x) s += jbar[f];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
+    mean = t / n_cells;
+  }
+  __syncthreads();
+  for (int f = threadIdx.x; f < n_cells; f += blockDim.x)
+    resid[f] = (E_np1[f] - E_n[f]) / dt + jbar[f] - mean;
+}
+
+// Getter: un-permute to the original order.  Any output may be NULL.
+template <typename T>
+__global__ void unpermute_kernel(long long n, const uint32_t* __restrict__ id,
+                                 const T* __restrict__ xi, const T* __restrict__ v,
+                                 const int32_t* __restrict__ cell, double dx, double* x_out,
+                                 double* v_out, int32_t* cell_out, double* xi_out) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const uint32_t j = id[i];
+    const double o = (double)xi[i];
+    const int32_t c = cell[i];
+    if (x_out) x_out[j] = ((double)c + o) * dx;
+    if (v_out) v_out[j] = (double)v[i];
+    if (cell_out) cell_out[j] = c;
+    if (xi_out) xi_out[j] = o;
+  }
+}
+
+static __global__ void unpermute_counts_kernel(long long n, const uint32_t* __restrict__ id,
+                                        const uint32_t* __restrict__ a, const uint32_t* __restrict__ b,
+                                        uint32_t* a_out, uint32_t* b_out) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const uint32_t j = id[i];
+    if (a_out) a_out[j] = a[i];
+    if (b_out) b_out[j] = b[i];
+  }
+}
+
+// sum_p v_p^2 (fp64), one atomic per block.
+template <typename T>
+__global__ void sumsq_kernel(long long n, const T* __restrict__ v, double* __restrict__ out) {
+  __shared__ double red[32];
+  double s = 0.0;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const double t = (double)v[i];
+    s += t * t;
+  }
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
+    atomicAdd(out, t);
+  }
+}
+
+// rho on cell centres, quadratic B-spline (A-10): with p = xi in [0,1] inside cell c the
+// weights on cells c-1, c, c+1 are (1-p)^2/2, 3/4 - (p-1/2)^2, p^2/2.
+template <typename T>
+__global__ void rho_kernel(long long n, const T* __restrict__ xi, const int32_t* __restrict__ cell,
+                           int32_t n_cells, double w_over_dx, double* __restrict__ rho) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const double p = (double)xi[i];
+    const int32_t c = cell[i];
+    const int32_t cl = c == 0 ? n_cells - 1 : c - 1;
+    const int32_t cr = c + 1 == n_cells ? 0 : c + 1;
+    atomicAdd(&rho[cl], w_over_dx * 0.5 * (1.0 - p) * (1.0 - p));
+    atomicAdd(&rho[c], w_over_dx * (0.75 - (p - 0.5) * (p - 0.5)));
+    atomicAdd(&rho[cr], w_over_dx * 0.5 * p * p);
+  }
+}
+
+}  // namespace picb200

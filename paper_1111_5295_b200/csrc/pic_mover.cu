@@ -1,0 +1,123 @@
+// pic_mover.cu — launch side of the mover kernel (mover.cuh): launch shape, shared-memory
+// budget, argument packing.  SURVEY.md 8(a) a0-a8.
+#include <algorithm>
+#include <cmath>
+
+#include "mover.cuh"
+#include "pic_internal.h"
+
+namespace picb200 {
+
+namespace {
+
+template <typename T, bool D, bool G>
+cudaError_t set_smem(size_t bytes) {
+  return cudaFuncSetAttribute(mover_kernel<T, D, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)bytes);
+}
+
+template <typename T>
+cudaError_t set_smem_all(size_t bytes) {
+  cudaError_t e;
+  if ((e = set_smem<T, true, false>(bytes)) != cudaSuccess) return e;
+  if ((e = set_smem<T, true, true>(bytes)) != cudaSuccess) return e;
+  if ((e = set_smem<T, false, false>(bytes)) != cudaSuccess) return e;
+  return set_smem<T, false, true>(bytes);
+}
+
+template <typename T, bool D, bool G>
+int occupancy(size_t bytes) {
+  int nb = 0;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, D, G>, kBlock, bytes);
+  return nb;
+}
+
+template <typename T>
+void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const double* dE_np1,
+              double dt, double tol, int row0, int s) {
+  const pic_params& P = h->params;
+  const double dx = h->grid.length / h->grid.n_cells;
+  MoverArgs<T> a;
+  a.n = S.n;
+  a.xi0 = (const T*)S.xi[h->cur];
+  a.v0 = (const T*)S.v[h->cur];
+  a.cell0 = S.cell[h->cur];
+  const bool store = !(P.flags & PIC_FLAG_NO_STORE);
+  a.xi1 = store ? (T*)S.xi[1 - h->cur] : nullptr;
+  a.v1 = store ? (T*)S.v[1 - h->cur] : nullptr;
+  a.cell1 = store ? S.cell[1 - h->cur] : nullptr;
+  const bool counts = (P.flags & PIC_FLAG_COUNTS) && S.nsub;
+  a.nsub_out = counts ? S.nsub : nullptr;
+  a.ncross_out = counts ? S.ncross : nullptr;
+  a.E_n = dE_n;
+  a.E_np1 = dE_np1;
+  a.n_cells = h->grid.n_cells;
+  a.max_substeps = P.max_substeps;
+  a.picard_max = P.picard_max;
+  a.tile = S.tile;
+  a.refill_threshold = 4;
+  a.qm_over_dx = S.q_over_m / dx;
+  a.dx = (T)dx;
+  a.inv_dx = (T)(1.0 / dx);
+  a.c_abs = (T)std::sqrt(2.0 * P.eps_a / dx);
+  a.c_rel = (T)(2.0 * P.eps_r);
+  a.c_cap = (T)std::sqrt(4.0 * P.kappa_max);
+  a.dt = (T)dt;
+  // a Picard tolerance below a few ulp of the kernel precision can never be met (A-3)
+  const double tol_floor = 4.0 * (sizeof(T) == 4 ? 1.1920929e-7 : 2.220446049250313e-16);
+  a.tol = (T)std::max(tol, tol_floor);
+  a.scale = S.w_q / dt;
+  a.partial = h->d_partial + (size_t)row0 * h->grid.n_cells;
+  a.queue = h->d_queue + s;
+  a.stats = h->d_stats;
+  const bool direct = P.cn_mode == PIC_CN_DIRECT;
+  const bool diag = (P.flags & PIC_FLAG_DIAG) != 0;
+  dim3 g(S.grid_blocks), b(kBlock);
+  if (direct && !diag) mover_kernel<T, true, false><<<g, b, h->smem_bytes, h->stream>>>(a);
+  else if (direct) mover_kernel<T, true, true><<<g, b, h->smem_bytes, h->stream>>>(a);
+  else if (!diag) mover_kernel<T, false, false><<<g, b, h->smem_bytes, h->stream>>>(a);
+  else mover_kernel<T, false, true><<<g, b, h->smem_bytes, h->stream>>>(a);
+}
+
+}  // namespace
+
+// Shared-memory budget and launch shape.  The whole grid is staged per block (SURVEY hard part
+// 6): n_cells * (8 + sizeof(T)) bytes; B200 allows 227 KB per block.
+int mover_configure(pic_handle* h) {
+  const size_t bytes = (size_t)h->grid.n_cells * (8 + h->elem);
+  if (bytes > 200 * 1024) return set_err(h, PIC_ERR_UNSUPPORTED, "n_cells too large for smem grid");
+  h->smem_bytes = bytes;
+  cudaError_t e = h->elem == 4 ? set_smem_all<float>(bytes) : set_smem_all<double>(bytes);
+  if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "cudaFuncSetAttribute(smem)", e);
+  int occ = h->elem == 4 ? occupancy<float, true, false>(bytes) : occupancy<double, true, false>(bytes);
+  if (occ < 1) return set_err(h, PIC_ERR_CUDA, "mover kernel does not fit on an SM");
+  h->blocks_per_sm = occ;
+  int rows = 0;
+  for (auto& S : h->sp) {
+    // persistent grid: one wave of resident blocks (a multiple of the SM count), fewer for
+    // small problems so that every warp still gets a few refills' worth of particles.
+    const long long full = (long long)h->sm_count * occ;
+    const long long want = (S.n + kBlock * 4 - 1) / (kBlock * 4);
+    S.grid_blocks = (int)std::max<long long>(1, std::min(full, want));
+    const long long warps = (long long)S.grid_blocks * (kBlock / 32);
+    long long tile = S.n / (warps * 8);                 // >= 8 claims per warp
+    tile = std::max<long long>(32, std::min<long long>(1024, tile / 32 * 32));
+    S.tile = (int)tile;
+    rows += S.grid_blocks;
+  }
+  h->total_rows = rows;
+  return PIC_OK;
+}
+
+int launch_mover(pic_handle* h, int s, const double* dE_n, const double* dE_np1, double dt,
+                 double tol, int row0) {
+  const SpeciesState& S = h->sp[s];
+  if (h->elem == 4) launch_t<float>(h, S, dE_n, dE_np1, dt, tol, row0, s);
+  else launch_t<double>(h, S, dE_n, dE_np1, dt, tol, row0, s);
+  h->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "mover_kernel launch", e);
+  return PIC_OK;
+}
+
+}  // namespace picb200
