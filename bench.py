@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""bench.py — mover throughput on BASELINE.json's metric workload (configs[2]: 4,096 cells,
+1e8 electrons, 16-mode field, dt = 10, fp32 mover), one JSON line on stdout.
+
+A "step" is one pass of the whole hot path = one pic_move_accumulate call
+over every particle.  `value` = particle sub-steps/s with everything resident in HBM (E and jbar
+are device arrays); `e2e` = the same through the C-ABI with HOST grid buffers (E^n, E^{n+1} copied
+host->device and jbar device->host inside the timed region; the particles are enslaved state that
+never leaves the GPU).  `roofline` is the plain-ALU FP32 roofline with the
+algorithmic op table of DESIGN.md 6; `cpu_baseline` is the oracle, as it stands, on a bounded
+sample.  `--impl reference` times the oracle alone (the reference arm of this tier).
+
+N > 1 (torchrun): independent replicas with different seeds, no data-path collective
+("replicas only"); value = total sub-steps of all ranks / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1111_5295_b200 import workloads as W  # noqa: E402
+
+METRIC = "mover_particle_substeps_per_s"
+UNIT = "sub-steps/s"
+# Algorithmic op table (paper's convention: every FP / int / SF thread-operation = 1, FMA = 2;
+# P:94-105), SURVEY 8(d) / DESIGN.md 6: per in-cell sub-step and per crossing sub-step.
+OPS_INCELL, OPS_CROSS = 43.0, 72.0
+
+
+def _workload(name, n, seed):
+    if name == "cfg2":
+        return W.config2(n=n or 100_000_000, seed=seed)
+    if name == "cfg3":
+        return W.config3(n=n or 20_000_000, seed=seed)
+    if name == "cfg0":
+        return W.config0(n=n or 6400, seed=seed)
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler(threading.Thread):
+    """SM clock / throttle-reason samples during the timed region (pynvml, 20 ms period)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self._stop_ev = threading.Event()
+        try:
+            import pynvml as N
+            N.nvmlInit()
+            self.N = N
+            self.h = N.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = N.nvmlDeviceGetMaxClockInfo(self.h, N.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        N = self.N
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40,
+                 "sw_thermal_slowdown": 0x20, "hw_power_brake": 0x80}
+        while not self._stop_ev.is_set():
+            try:
+                self.samples.append(N.nvmlDeviceGetClockInfo(self.h, N.NVML_CLOCK_SM))
+                try:
+                    r = N.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:  # noqa: BLE001
+                    r = N.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:  # noqa: BLE001
+                pass
+            time.sleep(0.02)
+
+    def stop(self):
+        self._stop_ev.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def oracle_rate(cfg, sample, threads=1):
+    """Time the oracle, as it stands (serial, fp64, Picard), on the first `sample` particles."""
+    from oracle import pic_oracle as o
+    o.build()
+    sp = cfg["species"][0]
+    n = min(sample, sp["x"].shape[0])
+    c, s = o.bin_particles(cfg["n_cells"], cfg["length"], sp["x"][:n])
+    t0 = time.perf_counter()
+    r = o.move_accumulate(cfg["n_cells"], cfg["length"], sp["q_over_m"], sp["w_q"], c, s,
+                          sp["v"][:n], cfg["E_n"], cfg["E_np1"], cfg["dt"],
+                          o.make_params(tol=cfg.get("tol", 1e-10)), want_state=False)
+    dt = time.perf_counter() - t0
+    return r["stats"].n_sub / dt, r["stats"].n_sub, dt, n
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores, bounded sample per step."""
+    if rank != 0:
+        return
+    sample = args.ref_sample
+    cfg = _workload(args.workload, sample, args.seed)
+    for _ in range(args.warmup):
+        oracle_rate(cfg, min(sample, 1 << 14))
+    tot_sub, tot_t = 0, 0.0
+    for _ in range(args.steps):
+        _, nsub, dt, n = oracle_rate(cfg, sample)
+        tot_sub += nsub
+        tot_t += dt
+    val = tot_sub / tot_t
+    sample_desc = f"first {n} particles of {args.workload} per step, serial fp64 oracle (Picard)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": args.workload, "sample_particles": n},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": sample_desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg2", "cfg3"])
+    ap.add_argument("--n", type=int, default=0, help="override the particle count (debug)")
+    ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
+    ap.add_argument("--cn-mode", default="direct", choices=["direct", "picard"])
+    ap.add_argument("--seed", type=int, default=W.DEFAULT_SEED)
+    ap.add_argument("--cpu-sample", type=int, default=1 << 22)
+    ap.add_argument("--ref-sample", type=int, default=1 << 19)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1111_5295_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    B.load()
+
+    # replicas only: every rank runs its own copy of the workload with its own seed
+    cfg = _workload(args.workload, args.n, args.seed + rank)
+    sp = cfg["species"][0]
+    n_p = sp["x"].shape[0]
+    stream = torch.cuda.current_stream().cuda_stream
+    pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=args.precision,
+                cn_mode=args.cn_mode, stream=stream)
+    ng = cfg["n_cells"]
+    dEn = torch.from_numpy(cfg["E_n"]).cuda()
+    dEp = torch.from_numpy(cfg["E_np1"]).cuda()
+    dj = torch.empty(ng, dtype=torch.float64, device="cuda")
+    hEn = torch.from_numpy(cfg["E_n"]).pin_memory()
+    hEp = torch.from_numpy(cfg["E_np1"]).pin_memory()
+    hj = torch.empty(ng, dtype=torch.float64).pin_memory()
+    dt, tol = cfg["dt"], cfg.get("tol", 1e-10)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+    torch.cuda.synchronize()
+    st0 = pic.get_stats()
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    st1 = pic.get_stats()
+    n_sub, n_cross = st1["n_sub"], st1["n_cross"]        # per step (state n is constant)
+    launches = st1["n_launches"] - st0["n_launches"]
+
+    # ---- end to end: host E^n, E^{n+1} in, host jbar out, every step
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        pic.move_accumulate(hEn.numpy(), hEp.numpy(), dt, tol, jbar_out=hj.numpy())
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+
+    # ---- dominant kernel alone: CUDA events around the mover launches (library-side events)
+    kms = []
+    for _ in range(min(args.steps, 5)):
+        pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+        kms.append(pic.get_stats()["last_move_ms"])
+    k_ms = float(np.mean(kms))
+
+    if world > 1:
+        t = torch.tensor([ms, e2e_s, float(n_sub), float(n_cross)], dtype=torch.float64, device="cuda")
+        tmax = t.clone()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone()
+        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms, e2e_s = float(tmax[0]), float(tmax[1])
+        tot_sub, tot_cross = float(tsum[2]), float(tsum[3])
+    else:
+        tot_sub, tot_cross = float(n_sub), float(n_cross)
+    if rank != 0:
+        pic.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = tot_sub * args.steps / (ms * 1e-3)
+    e2e = tot_sub * args.steps / e2e_s
+    props = torch.cuda.get_device_properties(local_rank)
+    sms = props.multi_processor_count
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:  # noqa: BLE001
+        pass
+    sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    if args.precision == "fp32":
+        peak_gops = sms * 128 * 2 * sm_max_mhz * 1e-3      # Eq. 1: lanes x 2 (FMA) x clock
+    else:
+        peak_gops = sms * 64 * 2 * sm_max_mhz * 1e-3       # FP64: 64 DFMA lanes per SM
+    ops_per_launch = OPS_INCELL * (n_sub - n_cross) + OPS_CROSS * n_cross
+    achieved = ops_per_launch / (k_ms * 1e-3) * 1e-9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if args.precision == "fp32" else "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {ng} cells, {n_p} particles/GPU, dt={dt}",
+                   "precision": args.precision, "cn_mode": args.cn_mode,
+                   "substeps_per_particle": n_sub / max(n_p, 1),
+                   "crossing_fraction": n_cross / max(n_sub, 1),
+                   "l2": "inputs larger than L2 (particle state %.0f MB/GPU)" % (n_p * 12e-6),
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "gop_per_s_model": value * ops_per_launch / max(n_sub, 1) * 1e-9,
+        "clocks": clocks,
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 2 * ng * 8,
+                "d2h_bytes_per_step": ng * 8},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_gops, "unit": "GOp/s",
+                     "frac": achieved / peak_gops, "traffic": None,
+                     "kernel": "mover_kernel", "kernel_ms": k_ms,
+                     "ops_per_launch": ops_per_launch,
+                     "peak_source": "derived: SMs x lanes x 2 x sm_max_mhz (DESIGN.md 6)",
+                     "hbm_gbs_algorithmic": n_p * (24 if args.precision == "fp32" else 40) / (k_ms * 1e-3) * 1e-9},
+    }
+    if not args.no_cpu_baseline:
+        rate, nsub_s, dts, ns = oracle_rate(cfg, args.cpu_sample)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"first {ns} particles of {args.workload} "
+                                          f"({nsub_s} sub-steps, {dts:.1f} s), serial fp64 oracle"}
+    print(json.dumps(line), flush=True)
+    pic.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,225 @@
+"""`-m gpu` parity tests: the CUDA path (through the C-ABI) against the oracle, element by
+element on the same seeded inputs, with the tolerances of BASELINE.json's north_star:
+fp64 rel L2 1e-10 on jbar, x, v; fp32 1e-4 on jbar, 1e-5 on x, v, continuity 1e-5 relative.
+Branch-flipped particles (SURVEY A-12) are excluded, counted and reported."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1111_5295_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def G():
+    import gpu_helpers
+    from paper_1111_5295_b200 import binding
+    binding.load()
+    return gpu_helpers
+
+
+def _report(name, m):
+    print(f"[parity] {name}: x={max(m['x']):.2e} v={max(m['v']):.2e} j={m['j']:.2e} "
+          f"cont={m['cont']:.2e} flips={m['flips']}/{m['n']} "
+          f"sub={m['stats']['n_sub']} cross={m['stats']['n_cross']}")
+
+
+# ---- configs[0]: 6,400 electrons, 64 cells, dt = 0.5 ------------------------------------------
+@pytest.mark.parametrize("precision,cn_mode", [("fp64", "picard"), ("fp64", "direct"),
+                                               ("fp32", "direct"), ("fp32", "picard")])
+def test_cfg0_parity(G, oracle, precision, cn_mode):
+    cfg = W.config0()
+    m = G.parity(oracle, cfg, precision, cn_mode)
+    _report(f"cfg0 {precision} {cn_mode}", m)
+    G.assert_parity(m, precision)
+    if precision == "fp64":
+        assert m["flips"] == 0
+        assert m["stats"]["n_sub"] == m["ostats"]["n_sub"]
+        assert m["stats"]["n_cross"] == m["ostats"]["n_cross"]
+    m["gpu"]["pic"].close()
+
+
+# ---- configs[2] / [3] shapes at sizes the oracle finishes in seconds (several tiles + a
+# ragged tail: 200,003 is not a multiple of 32) --------------------------------------------------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_cfg2_small_parity(G, oracle, precision):
+    cfg = W.config2(n=200_003)
+    m = G.parity(oracle, cfg, precision)
+    _report(f"cfg2/200k {precision}", m)
+    G.assert_parity(m, precision)
+    assert m["stats"]["n_sub"] > 20 * 200_003   # paper-shaped: tens of sub-steps per particle
+    m["gpu"]["pic"].close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_cfg3_small_invariants(G, oracle, precision):
+    """configs[3] orbits are sensitive: gate on flips-excluded fp64 parity and
+    on the invariants; fp32 per-particle parity is reported, continuity is gated."""
+    cfg = W.config3(n=20_011)
+    m = G.parity(oracle, cfg, precision)
+    _report(f"cfg3/20k {precision}", m)
+    if precision == "fp64":
+        G.assert_parity(m, "fp64", max_flip_frac=5e-3)
+    else:
+        assert m["cont"] <= G.TOL["fp32"]["cont"]
+        assert m["flips"] <= 0.05 * m["n"]
+    assert m["stats"]["n_substep_cap"] == 0
+    m["gpu"]["pic"].close()
+
+
+# ---- two species (IAW shape, small), multi-species sum of jbar ---------------------------------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_two_species_parity(G, oracle, precision):
+    cfg = W.config1(ppc=40)
+    xf = W.face_positions(cfg["n_cells"], cfg["length"])
+    cfg["E_n"] = 0.02 * np.sin(2 * math.pi * xf / cfg["length"])
+    cfg["E_np1"] = 0.02 * np.sin(2 * math.pi * xf / cfg["length"] + 0.2)
+    m = G.parity(oracle, cfg, precision)
+    _report(f"iaw-small {precision}", m)
+    G.assert_parity(m, precision)
+    m["gpu"]["pic"].close()
+
+
+# ---- closed forms on the GPU (the oracle's pins P-1, P-2 applied to the kernel) ----------------
+@pytest.mark.parametrize("precision,tol", [("fp64", 1e-12), ("fp32", 2e-5)])
+def test_free_streaming_and_uniform_field(G, precision, tol):
+    n_cells, length, dt = 32, 10.0, 2.5
+    n = 1000
+    x = W.uniform01(11, 1, n) * length * (1 - 1e-12)
+    v = W.normal01(11, 2, n)
+    dx = length / n_cells
+    for E0 in (0.0, 0.3):
+        E = np.full(n_cells, E0)
+        cfg = dict(n_cells=n_cells, length=length, dt=dt, tol=1e-12, E_n=E, E_np1=E,
+                   species=[dict(name="e", q_over_m=-1.0, w_q=-length / n, x=x, v=v)])
+        g = G.gpu_run(cfg, precision)
+        s = g["species"][0]
+        a = -E0
+        X0 = (s["cell0"] + s["xi0"]) * dx          # the (possibly fp32-rounded) start
+        X1 = X0 + s["v0"] * dt + 0.5 * a * dt * dt
+        d = np.abs(((s["x"] - X1 + length / 2) % length) - length / 2)
+        assert d.max() < tol * 10, (E0, d.max())
+        assert np.max(np.abs(s["v"] - (s["v0"] + a * dt))) < tol * 10
+        # P-8: sum_f J_f = w_q sum_p (X1 - X0)  <=>  sum_f jbar_f = w_q sum (X1-X0)/(dt dx)
+        lhs = g["jbar"].sum()
+        rhs = (-length / n) * np.sum(s["v0"] * dt + 0.5 * a * dt * dt) / (dt * dx)
+        assert abs(lhs - rhs) <= (1e-11 if precision == "fp64" else 2e-5) * max(abs(rhs), 1.0)
+        g["pic"].close()
+
+
+# ---- edge cases --------------------------------------------------------------------------------
+def test_edge_cases(G, oracle):
+    n_cells, length = 8, 4.0
+    dx = length / n_cells
+    xf = W.face_positions(n_cells, length)
+    E = 0.5 * np.sin(2 * math.pi * xf / length)
+    # particles exactly on faces (A-5), at 0, just below L, zero velocity, and a single particle
+    x = np.array([0.0, dx, 3 * dx, np.nextafter(length, 0.0), 1.3, 2.0, 0.25])
+    v = np.array([1.0, -1.0, 0.0, 2.0, 0.0, -3.0, 1e-9])
+    cfg = dict(n_cells=n_cells, length=length, dt=1.7, tol=1e-12, E_n=E, E_np1=0.9 * E,
+               species=[dict(name="e", q_over_m=-1.0, w_q=-0.5, x=x, v=v)])
+    for cn in ("picard", "direct"):
+        m = G.parity(oracle, cfg, "fp64", cn)
+        _report(f"edge fp64 {cn}", m)
+        G.assert_parity(m, "fp64", max_flip_frac=0.0)
+        m["gpu"]["pic"].close()
+    m = G.parity(oracle, cfg, "fp32")
+    assert m["cont"] < 1e-5
+    m["gpu"]["pic"].close()
+    # one cell only: both faces are face 0
+    cfg1 = dict(n_cells=1, length=1.0, dt=0.9, tol=1e-12, E_n=np.array([0.3]),
+                E_np1=np.array([0.1]),
+                species=[dict(name="e", q_over_m=1.0, w_q=1.0, x=np.array([0.2, 0.7]),
+                              v=np.array([1.5, -2.5]))])
+    m = G.parity(oracle, cfg1, "fp64")
+    G.assert_parity(m, "fp64", max_flip_frac=0.0)
+    m["gpu"]["pic"].close()
+
+
+def test_empty_species_and_bad_input(G):
+    from paper_1111_5295_b200 import binding as B
+    n_cells, length = 16, 8.0
+    E = np.zeros(n_cells)
+    e = np.empty(0)
+    pic = B.Pic(n_cells, length, [dict(q_over_m=-1.0, w_q=-1.0, x=e, v=e)], precision="fp32")
+    j = pic.move_accumulate(E, E, 1.0)
+    assert np.all(j == 0.0) and pic.get_stats()["n_sub"] == 0
+    pic.close()
+    with pytest.raises(B.PicError):   # x outside [0, L)
+        B.Pic(n_cells, length, [dict(q_over_m=-1.0, w_q=-1.0, x=np.array([8.5]), v=np.array([0.0]))])
+    with pytest.raises(B.PicError):   # non-finite v
+        B.Pic(n_cells, length, [dict(q_over_m=-1.0, w_q=-1.0, x=np.array([1.0]), v=np.array([np.nan]))])
+
+
+def test_substep_cap_is_reported(G):
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config0(n=640)
+    sp = cfg["species"][0]
+    pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp64", max_substeps=2)
+    with pytest.raises(B.PicError) as ei:
+        pic._chk(pic._L.pic_move_accumulate(pic._h, B._ptr(cfg["E_n"]), B._ptr(cfg["E_np1"]),
+                                            B.C.c_double(cfg["dt"]), B.C.c_double(1e-10),
+                                            B._ptr(np.empty(cfg["n_cells"]))))
+    assert ei.value.code == B.PIC_ERR_SUBSTEP_CAP
+    assert pic.get_stats()["n_substep_cap"] > 0
+    pic.close()
+
+
+# ---- boundary: residual, repeatability, device pointers, commit ---------------------------------
+def test_residual_repeat_commit(G, oracle):
+    import torch
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config0()
+    sp = cfg["species"][0]
+    pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp64", cn_mode="picard",
+                flags=B.PIC_FLAG_COUNTS, stream=torch.cuda.current_stream().cuda_stream)
+    dt = cfg["dt"]
+    j1 = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], dt)
+    j2 = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], dt)     # state n untouched: repeatable
+    assert np.max(np.abs(j1 - j2)) <= 1e-13 * np.max(np.abs(j1))
+    # device pointers in, device pointer out (no host copies inside the call)
+    dEn = torch.from_numpy(cfg["E_n"]).cuda()
+    dEp = torch.from_numpy(cfg["E_np1"]).cuda()
+    dj = torch.empty(cfg["n_cells"], dtype=torch.float64, device="cuda")
+    pic.move_accumulate(dEn, dEp, dt, jbar_out=dj)
+    torch.cuda.synchronize()
+    assert np.max(np.abs(dj.cpu().numpy() - j1)) <= 1e-13 * np.max(np.abs(j1))
+    # a9 against the oracle's residual of the oracle's jbar
+    pic.set_step(cfg["E_n"], dt)
+    R = pic.residual(cfg["E_np1"])
+    ref = G.oracle_run(oracle, cfg)
+    Rref = oracle.residual(cfg["E_n"], cfg["E_np1"], dt, ref["jbar"])
+    assert G.rel_l2(R, Rref) < 1e-10
+    # P-12: sum_f R_f = sum_f (E^{n+1} - E^n)/dt
+    assert abs(R.sum() - (cfg["E_np1"] - cfg["E_n"]).sum() / dt) < 1e-12
+    # commit: state n+1 becomes state n (re-binned); a second move must match the oracle
+    # continuing from its own n+1 state
+    r1 = ref["species"][0]
+    pic.commit()
+    got = pic.get_particles(0, B.PIC_STATE_N)
+    assert np.array_equal(got["cell"], r1["cell"])
+    j3 = pic.move_accumulate(cfg["E_np1"], cfg["E_np1"], dt)
+    cfgb = dict(cfg, E_n=cfg["E_np1"])
+    ref2 = G.oracle_run(oracle, cfgb, state=[(r1["cell"], r1["s"], r1["v"])])
+    assert G.rel_l2(j3, ref2["jbar"]) < 1e-9
+    after = pic.get_particles(0, B.PIC_STATE_NP1)
+    assert G.rel_l2(after["v"], ref2["species"][0]["v"]) < 1e-9
+    pic.close()
+
+
+def test_energy_identity_on_gpu(G):
+    """P-9 on the kernel: sum_p w_m (v1^2 - v0^2)/2 = dt dx sum_f jbar_f E^{n+1/2}_f."""
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config2(n=100_000)
+    sp = cfg["species"][0]
+    dx = cfg["length"] / cfg["n_cells"]
+    for precision, tol in (("fp64", 1e-11), ("fp32", 1e-4)):
+        pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=precision)
+        jbar = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+        dK = pic.kinetic_energy(B.PIC_STATE_NP1)[0] - pic.kinetic_energy(B.PIC_STATE_N)[0]
+        work = cfg["dt"] * dx * np.sum(jbar * 0.5 * (cfg["E_n"] + cfg["E_np1"]))
+        print(f"[energy] {precision}: dK={dK:.6e} work={work:.6e} rel={(dK - work) / abs(work):.2e}")
+        assert abs(dK - work) <= tol * abs(work)
+        pic.close()
