@@ -134,7 +134,10 @@ def test_edge_cases(G, oracle):
                 species=[dict(name="e", q_over_m=1.0, w_q=1.0, x=np.array([0.2, 0.7]),
                               v=np.array([1.5, -2.5]))])
     m = G.parity(oracle, cfg1, "fp64")
-    G.assert_parity(m, "fp64", max_flip_frac=0.0)
+    # one cell: jbar_{c+1} - jbar_c = 0 identically, so the relative continuity metric has no
+    # denominator; check the absolute residual (rho is constant) and the rest as usual
+    assert m["cont_max"] < 1e-12 and m["flips"] == 0
+    assert max(m["x"]) < 1e-10 and max(m["v"]) < 1e-10 and m["j"] < 1e-10
     m["gpu"]["pic"].close()
 
 
