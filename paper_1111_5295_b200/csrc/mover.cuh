@@ -8,11 +8,16 @@
 // Shares no code with oracle/.  Design notes:
 //  * all per-particle arithmetic is in CELL UNITS: xi = (x - x_c)/dx in [0,1], u = v/dx,
 //    A_f = (q/m) E^{n+1/2}_f / dx.  Inside cell c: A(xi) = A_L + dA xi, dA = A_R - A_L = a'.
-//  * the deposit uses the telescoped per-cell-visit form of the per-sub-step sum (SURVEY P-7):
-//    a stay in one cell from xi_in to xi_out contributes delta*m to the right face and
-//    delta*(1-m) to the left face, delta = xi_out - xi_in, m = (xi_in + xi_out)/2 -- the sum of
-//    P:212's per-sub-step linear-spline deposits over that stay, to rounding.  It is flushed to
-//    shared memory on crossing / at orbit end (the paper's register accumulation).
+//  * deposit, two modes (template PER_VISIT):
+//      ENDPOINT (default): the per-sub-step linear-spline deposits of P:212 telescope exactly
+//      (SURVEY P-7): J_f = G(X1 - f) - G(X0 - f), G = running integral of the hat function, X
+//      unwrapped in cell units.  The sub-step loop only tracks k, the signed number of faces
+//      crossed; at orbit end the particle adds +-1 to every face it passed completely (an int32
+//      difference array in shared memory, native ATOMS.ADD, exact) and four fractional terms in
+//      fp64.  The block prefix-sums the difference array once at its flush.
+//      PER_VISIT: the paper's register accumulation: the stay in a cell from xi_in to
+//      xi_out is flushed to the two faces on crossing / at orbit end with shared-memory fp64
+//      atomics (a CAS loop on sm_100a: only 32-bit integer shared atomics are native).
 //  * divergence (variable sub-step counts): persistent warps; a lane whose
 //    orbit is finished parks its result and, once enough lanes of the warp are parked, the
 //    parked lanes store and pull the next particles of the warp's current index range
@@ -59,6 +64,13 @@ struct MoverArgs {
   unsigned long long* stats;   // [ST_COUNT] totals (accumulated)
 };
 
+// Dynamic shared memory of one block (bytes): F fp64 [n], A T [n+2] (halo), D int32 [n].
+template <typename T>
+__host__ __device__ inline size_t mover_smem_bytes(int n_cells) {
+  size_t b = (size_t)n_cells * (sizeof(double) + sizeof(int32_t)) + (size_t)(n_cells + 2) * sizeof(T);
+  return (b + 15) & ~(size_t)15;
+}
+
 // ---- precision-specific primitives -------------------------------------------------------
 template <typename T> struct Prim;
 
@@ -70,8 +82,6 @@ template <> struct Prim<float> {
   static __device__ __forceinline__ float sqrt(float x) {   // MUFU.SQRT
     float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
   static __device__ __forceinline__ float div(float a, float b) { return a * rcp(b); }
-  static __device__ __forceinline__ float tiny() { return 1e-30f; }
-  static __device__ __forceinline__ float eps() { return 1.1920929e-7f; }
 };
 
 template <> struct Prim<double> {
@@ -79,15 +89,14 @@ template <> struct Prim<double> {
   static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
   static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
   static __device__ __forceinline__ double div(double a, double b) { return a / b; }
-  static __device__ __forceinline__ double tiny() { return 1e-300; }
-  static __device__ __forceinline__ double eps() { return 2.220446049250313e-16; }
 };
 
 template <typename T> __device__ __forceinline__ T tabs(T x);
 template <> __device__ __forceinline__ float tabs<float>(float x) { return fabsf(x); }
 template <> __device__ __forceinline__ double tabs<double>(double x) { return fabs(x); }
-template <typename T> __device__ __forceinline__ T tmin(T a, T b) { return a < b ? a : b; }
-template <typename T> __device__ __forceinline__ T tmax(T a, T b) { return a > b ? a : b; }
+// IEEE min/max: a NaN operand is dropped (fmaxf(NaN, x) = x), which the estimator relies on.
+template <typename T> __device__ __forceinline__ T tmin(T a, T b);
+template <typename T> __device__ __forceinline__ T tmax(T a, T b);
 template <> __device__ __forceinline__ float tmin<float>(float a, float b) { return fminf(a, b); }
 template <> __device__ __forceinline__ float tmax<float>(float a, float b) { return fmaxf(a, b); }
 template <> __device__ __forceinline__ double tmin<double>(double a, double b) { return fmin(a, b); }
@@ -98,49 +107,91 @@ template <typename T>
 struct Lane {
   T xi, u, r;          // in-cell offset, velocity in cells/time, remaining time (O2)
   T AL, dA, cap;       // constants of the current cell (O3) and its kappa cap (A-2)
-  T xin;               // xi at entry into the current cell (telescoped deposit)
+  T xa;                // ENDPOINT: xi at the orbit start;  PER_VISIT: xi at entry into the cell
   int32_t c;           // cell
+  int32_t k;           // ENDPOINT: signed number of faces crossed so far
+  int32_t c0;          // ENDPOINT: start cell
   uint32_t ns, nc;     // sub-steps, crossings of this orbit
   long long idx;       // particle index; -1 = nothing parked
 };
 
-// O3: constants of cell c from the staged face values.
+// O3: constants of cell c.  sA carries a one-face halo on both sides: sA[f+1] = A_f,
+// sA[0] = A_{n-1}, sA[n+1] = A_0, so the two faces of cell c are sA[c+1], sA[c+2].
 template <typename T>
-__device__ __forceinline__ void load_cell(const T* __restrict__ sA, int32_t n_cells, T c_cap,
-                                          Lane<T>& p) {
-  const int32_t cr = (p.c + 1 == n_cells) ? 0 : p.c + 1;
-  const T AL = sA[p.c], AR = sA[cr];
+__device__ __forceinline__ void load_cell(const T* __restrict__ sA, T c_cap, Lane<T>& p) {
+  const T AL = sA[p.c + 1], AR = sA[p.c + 2];
   p.AL = AL;
   p.dA = AR - AL;
   // A-2: dtau <= sqrt(4 kappa_max / |a'|); |dA| = 0 gives +inf (no cap).
   p.cap = c_cap * Prim<T>::rsqrt(tabs(p.dA));
 }
 
-// a5/O8 (telescoped): flush the stay [xin, xout] in cell c to the block accumulators.
+// PER_VISIT a5/O8: flush the stay [xin, xout] in cell c to the block accumulators.
 template <typename T>
-__device__ __forceinline__ void deposit(double* __restrict__ sJ, int32_t n_cells, int32_t c,
-                                        T xin, T xout) {
+__device__ __forceinline__ void deposit_visit(double* __restrict__ sF, int32_t n_cells,
+                                              int32_t c, T xin, T xout) {
   const T delta = xout - xin;
   const T right = delta * (T(0.5) * (xin + xout));
   const T left = delta - right;
   const int32_t cr = (c + 1 == n_cells) ? 0 : c + 1;
-  atomicAdd(&sJ[c], (double)left);
-  atomicAdd(&sJ[cr], (double)right);
+  atomicAdd(&sF[c], (double)left);
+  atomicAdd(&sF[cr], (double)right);
+}
+
+// ENDPOINT a5/O8 (SURVEY P-7): J_f = G(X1 - f) - G(X0 - f) for a particle that went from
+// (c0, xi0) to (c1, xi1) crossing k faces (signed).  With g0(x) = 1 - (1-x)^2/2 (own left
+// face) and g1(x) = x^2/2 (own right face):
+//   J_f = [faces passed completely: +-1] + g0(xi1)[f=c1] + g1(xi1)[f=c1+1]
+//                                       - g0(xi0)[f=c0] - g1(xi0)[f=c0+1].
+// The +-1 run covers faces [c0, c0+k) for k > 0 and [c1, c1+|k|) for k < 0 (periodic); it goes
+// into the difference array sD (prefix-summed at the block flush), whole turns of the ring into
+// sD[0].
+__device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_t* __restrict__ sD,
+                                                 int32_t n, int32_t c0, double x0, int32_t c1,
+                                                 double x1, int32_t k) {
+  const int32_t c0r = (c0 + 1 == n) ? 0 : c0 + 1;
+  const int32_t c1r = (c1 + 1 == n) ? 0 : c1 + 1;
+  if (k == 0) {
+    // same cell: one term per face, no cancellation between atomics
+    const double d = x1 - x0, m = 0.5 * (x0 + x1);
+    atomicAdd(&sF[c0], d * (1.0 - m));
+    atomicAdd(&sF[c0r], d * m);
+    return;
+  }
+  atomicAdd(&sF[c1], 1.0 - 0.5 * (1.0 - x1) * (1.0 - x1));
+  atomicAdd(&sF[c1r], 0.5 * x1 * x1);
+  atomicAdd(&sF[c0], 0.5 * (1.0 - x0) * (1.0 - x0) - 1.0);
+  atomicAdd(&sF[c0r], -0.5 * x0 * x0);
+  const int32_t sgn = k > 0 ? 1 : -1;
+  int32_t len = k > 0 ? k : -k;
+  const int32_t a = k > 0 ? c0 : c1;
+  if (len >= n) {
+    const int32_t w = len / n;
+    len -= w * n;
+    atomicAdd(&sD[0], sgn * w);
+  }
+  if (len > 0) {
+    const int32_t e = a + len;
+    atomicAdd(&sD[a], sgn);
+    if (e < n) atomicAdd(&sD[e], -sgn);
+    else if (e > n) { atomicAdd(&sD[0], sgn); atomicAdd(&sD[e - n], -sgn); }
+  }
 }
 
 // One sub-step (O3-O8) of the lane's particle.  CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.
-template <typename T, bool CN_DIRECT, bool DIAG>
+template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT>
 __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restrict__ sA,
-                                        double* __restrict__ sJ, Lane<T>& p,
+                                        double* __restrict__ sF, Lane<T>& p,
                                         unsigned& picard_its, unsigned* diag) {
   // ---- a2 / O4: estimator (Eq. 6-8), L1 form, in cell units:
   //   alpha = dx (|A| + |dA u|)/2, beta = eps_r dx (|A| + |u|)
   //   dtau = max( sqrt(eps_a/alpha), beta/alpha ) = max( c_abs d, c_rel (|A|+|u|) d^2 ),
-  //   d = (|A| + |dA u|)^(-1/2)  (one rsqrt).  A-1: floor the sum at `tiny`.
+  //   d = (|A| + |dA u|)^(-1/2)  (one rsqrt).
+  // A-1 (alpha = 0): d = +inf, the first term is +inf and the second +inf or NaN; the IEEE
+  // max/min drop the NaN, so dtau = min(cap, r) -- the same limit as flooring alpha.
   const T A = fma(p.dA, p.xi, p.AL);
   const T absA = tabs(A);
-  const T S = tmax(absA + tabs(p.dA * p.u), Prim<T>::tiny());
-  const T d = Prim<T>::rsqrt(S);
+  const T d = Prim<T>::rsqrt(absA + tabs(p.dA * p.u));
   T dtau = tmax(a.c_abs * d, (a.c_rel * (absA + tabs(p.u))) * (d * d));
   if (DIAG && dtau > p.cap) diag[ST_KAPPA_CAP]++;
   dtau = tmin(tmin(dtau, p.cap), p.r);
@@ -174,14 +225,15 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
   const T xi1 = fma(T(0.5) * dtau, p.u + u1, p.xi);   // Eq. 9
 
   if (xi1 >= T(0) && xi1 <= T(1)) {
-    // ---- O6: accept (inclusive, A-5).  The deposit of this sub-step is carried by xin.
+    // ---- O6: accept (inclusive, A-5).
     p.xi = xi1;
     p.u = u1;
     p.r -= dtau;
   } else {
     // ---- a4 / O7: crossing.  Land on the face the tentative step left through.
     const bool right = xi1 > T(1);
-    const T dxi = right ? T(1) - p.xi : -p.xi;        // signed distance to that face
+    const T face = right ? T(1) : T(0);
+    const T dxi = face - p.xi;                        // signed distance to that face
     const T Am = fma(T(0.5) * p.dA, dxi, A);          // A at the midpoint of the truncated step
     T D = fma(T(2) * Am, dxi, p.u * p.u);             // Eq. 12 (energy principle)
     if (DIAG && D < T(0)) diag[ST_NEG_DISC]++;
@@ -189,37 +241,53 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     const T sq = Prim<T>::sqrt(D);
     const T uc = right ? sq : -sq;
     // Root of F(dtau) = (A_m/2) dtau^2 + u dtau - dxi.  A-6: 2 dxi/(u+uc) when moving
-    // towards the face, Eq. 13 (uc-u)/A_m otherwise; one reciprocal for both.
+    // towards the face (the common case), Eq. 13 (uc-u)/A_m otherwise.
     const bool toward = right ? (p.u > T(0)) : (p.u < T(0));
-    const T num = toward ? T(2) * dxi : uc - p.u;
-    const T den = toward ? p.u + uc : Am;
-    T dtc = Prim<T>::div(num, den);
-    if (!toward && Am == T(0)) dtc = dtau;
+    T dtc;
+    if (toward) {
+      dtc = Prim<T>::div(T(2) * dxi, p.u + uc);
+    } else {
+      dtc = (Am == T(0)) ? dtau : Prim<T>::div(uc - p.u, Am);
+    }
     if (DIAG && !(dtc >= T(0) && dtc <= dtau)) diag[ST_CLAMPED]++;
-    dtc = tmin(tmax(dtc, T(0)), dtau);                // NaN -> 0 (fmax/fmin drop the NaN)
-    // a5 / O8: flush this cell visit, then enter the neighbour on its near face.
-    deposit<T>(sJ, a.n_cells, p.c, p.xin, right ? T(1) : T(0));
-    p.c = right ? ((p.c + 1 == a.n_cells) ? 0 : p.c + 1) : ((p.c == 0) ? a.n_cells - 1 : p.c - 1);
-    p.xi = right ? T(0) : T(1);
-    p.xin = p.xi;
+    dtc = tmin(tmax(dtc, T(0)), dtau);                // NaN -> 0 (IEEE max/min drop the NaN)
+    // a5: PER_VISIT flushes this cell visit now; ENDPOINT only counts the face.
+    if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, face);
+    else p.k += right ? 1 : -1;
+    // enter the neighbour on its near face
+    int32_t cn = right ? p.c + 1 : p.c - 1;
+    cn = (cn == a.n_cells) ? 0 : cn;
+    cn = (cn < 0) ? a.n_cells - 1 : cn;
+    p.c = cn;
+    p.xi = T(1) - face;
+    if (PER_VISIT) p.xa = p.xi;
     p.u = uc;
     p.r -= dtc;
     p.nc++;
-    load_cell<T>(sA, a.n_cells, a.c_cap, p);
+    load_cell<T>(sA, a.c_cap, p);
   }
   p.ns++;
 }
 
-template <typename T, bool CN_DIRECT, bool DIAG>
-__global__ void __launch_bounds__(kBlock, 2) mover_kernel(const MoverArgs<T> a) {
+template <typename T> struct LaunchCfg { static constexpr int min_blocks = 2; };
+
+template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT>
+__global__ void __launch_bounds__(kBlock, LaunchCfg<T>::min_blocks)
+mover_kernel(const MoverArgs<T> a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double* sJ = reinterpret_cast<double*>(smem_raw);                 // [n_cells] accumulators
-  T* sA = reinterpret_cast<T*>(sJ + a.n_cells);                     // [n_cells] A on faces
+  double* sF = reinterpret_cast<double*>(smem_raw);                 // [n] fp64 accumulators
+  T* sA = reinterpret_cast<T*>(sF + a.n_cells);                     // [n+2] A on faces + halo
+  int32_t* sD = reinterpret_cast<int32_t*>(sA + a.n_cells + 2);     // [n] difference array
+  __shared__ int32_t s_wtot[kBlock / 32];
 
   // ---- a0: field prologue.  E^{n+1/2} = (E^n + E^{n+1})/2 (north_star; A-11), A = (q/m)E/dx.
   for (int f = threadIdx.x; f < a.n_cells; f += blockDim.x) {
-    sA[f] = (T)(a.qm_over_dx * (0.5 * (a.E_n[f] + a.E_np1[f])));
-    sJ[f] = 0.0;
+    const T Af = (T)(a.qm_over_dx * (0.5 * (a.E_n[f] + a.E_np1[f])));
+    sA[f + 1] = Af;
+    if (f == 0) sA[a.n_cells + 1] = Af;
+    if (f == a.n_cells - 1) sA[0] = Af;
+    sF[f] = 0.0;
+    sD[f] = 0;
   }
   __syncthreads();
 
@@ -230,8 +298,8 @@ __global__ void __launch_bounds__(kBlock, 2) mover_kernel(const MoverArgs<T> a) 
   bool active = false;
   Lane<T> p;
   p.idx = -1;
-  p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xin = T(0);
-  p.c = 0; p.ns = p.nc = 0;
+  p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xa = T(0);
+  p.c = p.k = p.c0 = 0; p.ns = p.nc = 0;
   unsigned long long tot_sub = 0, tot_cross = 0, tot_pic = 0;
   unsigned picard_its = 0;
   unsigned diag[ST_COUNT];
@@ -254,9 +322,10 @@ __global__ void __launch_bounds__(kBlock, 2) mover_kernel(const MoverArgs<T> a) 
           else { next = (long long)t; end = next + a.tile < a.n ? next + a.tile : a.n; }
         }
         if (!active) {
-          // ---- a7: store the parked result (state n+1) ...
+          // ---- a7: store the parked result (state n+1) and deposit its current ...
           if (p.idx >= 0) {
-            deposit<T>(sJ, a.n_cells, p.c, p.xin, p.xi);   // last, partial cell visit
+            if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, p.xi);
+            else deposit_endpoint(sF, sD, a.n_cells, p.c0, (double)p.xa, p.c, (double)p.xi, p.k);
             if (a.xi1) {
               a.xi1[p.idx] = p.xi;
               a.v1[p.idx] = p.u * a.dx;
@@ -276,9 +345,11 @@ __global__ void __launch_bounds__(kBlock, 2) mover_kernel(const MoverArgs<T> a) 
             p.u = a.v0[cand] * a.inv_dx;
             p.c = a.cell0[cand];
             p.r = a.dt;
-            p.xin = p.xi;
+            p.xa = p.xi;
+            p.c0 = p.c;
+            p.k = 0;
             p.ns = 0; p.nc = 0;
-            load_cell<T>(sA, a.n_cells, a.c_cap, p);
+            load_cell<T>(sA, a.c_cap, p);
             active = p.r > T(0);
           }
         }
@@ -287,7 +358,7 @@ __global__ void __launch_bounds__(kBlock, 2) mover_kernel(const MoverArgs<T> a) 
       }
     }
     if (active) {
-      substep<T, CN_DIRECT, DIAG>(a, sA, sJ, p, picard_its, diag);
+      substep<T, CN_DIRECT, DIAG, PER_VISIT>(a, sA, sF, p, picard_its, diag);
       active = (p.r > T(0)) && (p.ns < (uint32_t)a.max_substeps);
     }
   }
@@ -311,10 +382,30 @@ __global__ void __launch_bounds__(kBlock, 2) mover_kernel(const MoverArgs<T> a) 
     if (lane == 0 && v) atomicAdd(&a.stats[i], (unsigned long long)v);
   }
 
-  // ---- a8: one flush per block: scaled block sums -> this block's row of `partial`.
+  // ---- a8: one flush per block.  Inclusive prefix sum of the difference array over
+  // the faces (each thread owns a contiguous chunk), then scaled block sums -> this block's
+  // row of `partial`.
   __syncthreads();
+  const int per = (a.n_cells + (int)blockDim.x - 1) / (int)blockDim.x;
+  const int fb = min((int)threadIdx.x * per, a.n_cells), fe = min(fb + per, a.n_cells);
+  int32_t s = 0;
+  for (int f = fb; f < fe; ++f) s += sD[f];
+  int32_t inc = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int32_t t = __shfl_up_sync(kFull, inc, o);
+    if (lane >= o) inc += t;
+  }
+  const int wid = threadIdx.x >> 5;
+  if (lane == 31) s_wtot[wid] = inc;
+  __syncthreads();
+  int32_t run = inc - s;                       // exclusive within the warp
+  for (int w = 0; w < wid; ++w) run += s_wtot[w];
   double* row = a.partial + (size_t)blockIdx.x * a.n_cells;
-  for (int f = threadIdx.x; f < a.n_cells; f += blockDim.x) row[f] = a.scale * sJ[f];
+  for (int f = fb; f < fe; ++f) {
+    run += sD[f];
+    row[f] = a.scale * (sF[f] + (double)run);
+  }
 }
 
 }  // namespace picb200

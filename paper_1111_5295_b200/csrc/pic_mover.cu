@@ -10,25 +10,36 @@ namespace picb200 {
 
 namespace {
 
-template <typename T, bool D, bool G>
-cudaError_t set_smem(size_t bytes) {
-  return cudaFuncSetAttribute(mover_kernel<T, D, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)bytes);
+// Dispatch over the kernel's template switches (CN mode, diagnostics, deposit mode).
+template <typename T, typename F>
+auto with_kernel(bool direct, bool diag, bool per_visit, F&& f) {
+  const int key = (direct ? 4 : 0) | (diag ? 2 : 0) | (per_visit ? 1 : 0);
+  switch (key) {
+    case 0: return f(mover_kernel<T, false, false, false>);
+    case 1: return f(mover_kernel<T, false, false, true>);
+    case 2: return f(mover_kernel<T, false, true, false>);
+    case 3: return f(mover_kernel<T, false, true, true>);
+    case 4: return f(mover_kernel<T, true, false, false>);
+    case 5: return f(mover_kernel<T, true, false, true>);
+    case 6: return f(mover_kernel<T, true, true, false>);
+    default: return f(mover_kernel<T, true, true, true>);
+  }
 }
 
 template <typename T>
 cudaError_t set_smem_all(size_t bytes) {
-  cudaError_t e;
-  if ((e = set_smem<T, true, false>(bytes)) != cudaSuccess) return e;
-  if ((e = set_smem<T, true, true>(bytes)) != cudaSuccess) return e;
-  if ((e = set_smem<T, false, false>(bytes)) != cudaSuccess) return e;
-  return set_smem<T, false, true>(bytes);
+  cudaError_t e = cudaSuccess;
+  for (int key = 0; key < 8 && e == cudaSuccess; ++key)
+    e = with_kernel<T>(key & 4, key & 2, key & 1, [&](auto k) {
+      return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    });
+  return e;
 }
 
-template <typename T, bool D, bool G>
+template <typename T>
 int occupancy(size_t bytes) {
   int nb = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, D, G>, kBlock, bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, true, false, false>, kBlock, bytes);
   return nb;
 }
 
@@ -72,24 +83,27 @@ void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const do
   a.stats = h->d_stats;
   const bool direct = P.cn_mode == PIC_CN_DIRECT;
   const bool diag = (P.flags & PIC_FLAG_DIAG) != 0;
+  const bool per_visit = (P.flags & PIC_FLAG_DEPOSIT_PER_VISIT) != 0;
   dim3 g(S.grid_blocks), b(kBlock);
-  if (direct && !diag) mover_kernel<T, true, false><<<g, b, h->smem_bytes, h->stream>>>(a);
-  else if (direct) mover_kernel<T, true, true><<<g, b, h->smem_bytes, h->stream>>>(a);
-  else if (!diag) mover_kernel<T, false, false><<<g, b, h->smem_bytes, h->stream>>>(a);
-  else mover_kernel<T, false, true><<<g, b, h->smem_bytes, h->stream>>>(a);
+  with_kernel<T>(direct, diag, per_visit, [&](auto k) {
+    k<<<g, b, h->smem_bytes, h->stream>>>(a);
+    return cudaSuccess;
+  });
 }
 
 }  // namespace
 
 // Shared-memory budget and launch shape.  The whole grid is staged per block (SURVEY hard part
-// 6): n_cells * (8 + sizeof(T)) bytes; B200 allows 227 KB per block.
+// 6): n_cells * (8 + 4 + sizeof(T)) bytes (fp64 sums, int32 difference array, field + halo);
+// B200 allows 227 KB per block.
 int mover_configure(pic_handle* h) {
-  const size_t bytes = (size_t)h->grid.n_cells * (8 + h->elem);
-  if (bytes > 200 * 1024) return set_err(h, PIC_ERR_UNSUPPORTED, "n_cells too large for smem grid");
+  const size_t bytes = h->elem == 4 ? mover_smem_bytes<float>(h->grid.n_cells)
+                                    : mover_smem_bytes<double>(h->grid.n_cells);
+  if (bytes > 220 * 1024) return set_err(h, PIC_ERR_UNSUPPORTED, "n_cells too large for smem grid");
   h->smem_bytes = bytes;
   cudaError_t e = h->elem == 4 ? set_smem_all<float>(bytes) : set_smem_all<double>(bytes);
   if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "cudaFuncSetAttribute(smem)", e);
-  int occ = h->elem == 4 ? occupancy<float, true, false>(bytes) : occupancy<double, true, false>(bytes);
+  int occ = h->elem == 4 ? occupancy<float>(bytes) : occupancy<double>(bytes);
   if (occ < 1) return set_err(h, PIC_ERR_CUDA, "mover kernel does not fit on an SM");
   h->blocks_per_sm = occ;
   int rows = 0;

@@ -63,12 +63,13 @@ def sub_cfg(cfg, subset):
     return out
 
 
-def parity(o, cfg, precision, cn_mode="direct", oracle_params=None):
+def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=0):
     """Run both sides; return metrics (SURVEY 8(c) 'Parity metrics').  Particles whose
     (n_sub, n_cross, cell) differ are branch flips (A-12): excluded from x/v, counted, and
     jbar is then recomputed on both sides on the non-flipped subset."""
     dx = cfg["length"] / cfg["n_cells"]
-    g = gpu_run(cfg, precision, cn_mode)
+    flags = B.PIC_FLAG_COUNTS | B.PIC_FLAG_DIAG | extra_flags
+    g = gpu_run(cfg, precision, cn_mode, flags=flags)
     oc = sub_cfg(cfg, [slice(None)] * len(cfg["species"]))
     ref = oracle_run(o, oc, oracle_params, state=oracle_state_for(cfg, precision))
     m = dict(flips=0, n=0, x=[], v=[], stats=g["stats"], ostats=ref["stats"].as_dict())
@@ -87,7 +88,7 @@ def parity(o, cfg, precision, cn_mode="direct", oracle_params=None):
         gj, rj = g["jbar"], ref["jbar"]
     else:
         sub = [np.nonzero(k)[0] for k in keep]
-        g2 = gpu_run(cfg, precision, cn_mode, subset=sub)
+        g2 = gpu_run(cfg, precision, cn_mode, flags=flags, subset=sub)
         r2 = oracle_run(o, sub_cfg(cfg, sub), oracle_params,
                         state=oracle_state_for(cfg, precision, sub))
         gj, rj = g2["jbar"], r2["jbar"]

@@ -69,6 +69,40 @@ def test_cfg3_small_invariants(G, oracle, precision):
     m["gpu"]["pic"].close()
 
 
+# ---- the paper's per-cell-visit register accumulation as the deposit mode ------------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("which", ["cfg0", "cfg2"])
+def test_per_visit_deposit_parity(G, oracle, precision, which):
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config0() if which == "cfg0" else W.config2(n=100_001)
+    m = G.parity(oracle, cfg, precision, extra_flags=B.PIC_FLAG_DEPOSIT_PER_VISIT)
+    _report(f"{which} {precision} per-visit", m)
+    G.assert_parity(m, precision)
+    # and the two deposit modes agree with each other to rounding
+    g2 = G.gpu_run(cfg, precision)
+    assert G.rel_l2(m["gpu"]["jbar"], g2["jbar"]) < (1e-12 if precision == "fp64" else 1e-6)
+    m["gpu"]["pic"].close()
+    g2["pic"].close()
+
+
+# ---- long orbits: many wraps of the periodic ring (end-point deposit: whole turns) -----------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_ring_wraps(G, oracle, precision):
+    n_cells, length = 8, 4.0
+    xf = W.face_positions(n_cells, length)
+    E = 0.05 * np.sin(2 * math.pi * xf / length)
+    n = 257
+    x = W.uniform01(5, 1, n) * length * (1 - 1e-12)
+    v = 6.0 * W.normal01(5, 2, n)          # |v| dt / L up to ~10 turns either way
+    cfg = dict(n_cells=n_cells, length=length, dt=3.0, tol=1e-12, E_n=E, E_np1=E,
+               species=[dict(name="e", q_over_m=-1.0, w_q=-length / n, x=x, v=v)])
+    m = G.parity(oracle, cfg, precision)
+    _report(f"ring-wraps {precision}", m)
+    G.assert_parity(m, precision, max_flip_frac=0.02)
+    assert np.max(np.abs(m["ref"]["species"][0]["k"])) > 3 * n_cells   # really wrapped
+    m["gpu"]["pic"].close()
+
+
 # ---- two species (IAW shape, small), multi-species sum of jbar ---------------------------------
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_two_species_parity(G, oracle, precision):
