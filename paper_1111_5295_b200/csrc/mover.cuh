@@ -102,17 +102,33 @@ template <> __device__ __forceinline__ float tmax<float>(float a, float b) { ret
 template <> __device__ __forceinline__ double tmin<double>(double a, double b) { return fmin(a, b); }
 template <> __device__ __forceinline__ double tmax<double>(double a, double b) { return fmax(a, b); }
 
-// Per-lane particle registers.
+
+// Tuning constants of the warp scheduler inside the kernel.
+constexpr int kInner = 4;          // sub-step rounds between two refill votes
+constexpr int kCrossBatch = 1;     // pending crossings needed before the crossing block runs
+                                   // (1 = process at once)
+
+// Per-lane particle registers.  r > 0 <=> an orbit is in flight; r < 0 marks an orbit cut off
+// at max_substeps (A-9).
 template <typename T>
 struct Lane {
   T xi, u, r;          // in-cell offset, velocity in cells/time, remaining time (O2)
   T AL, dA, cap;       // constants of the current cell (O3) and its kappa cap (A-2)
+  T pdt;               // pending crossing: +dtau (right face) / -dtau (left face); 0 = none
   T xa;                // ENDPOINT: xi at the orbit start;  PER_VISIT: xi at entry into the cell
   int32_t c;           // cell
   int32_t k;           // ENDPOINT: signed number of faces crossed so far
   int32_t c0;          // ENDPOINT: start cell
   uint32_t ns, nc;     // sub-steps, crossings of this orbit
-  long long idx;       // particle index; -1 = nothing parked
+  uint32_t idx;        // particle index
+  bool have;           // a particle (in flight or parked) occupies the lane
+};
+
+// ENDPOINT: start-cell terms are collected in registers while consecutive particles of the lane
+// start in the same cell (they do: the state is binned by cell) and flushed when it changes.
+struct StartAcc {
+  double f0, f1;       // pending contributions to faces cell, cell+1
+  int32_t cell;        // -1 = empty
 };
 
 // O3: constants of cell c.  sA carries a one-face halo on both sides: sA[f+1] = A_f,
@@ -138,30 +154,41 @@ __device__ __forceinline__ void deposit_visit(double* __restrict__ sF, int32_t n
   atomicAdd(&sF[cr], (double)right);
 }
 
+__device__ __forceinline__ void flush_start(double* __restrict__ sF, int32_t n, StartAcc& s) {
+  if (s.cell >= 0) {
+    atomicAdd(&sF[s.cell], s.f0);
+    atomicAdd(&sF[(s.cell + 1 == n) ? 0 : s.cell + 1], s.f1);
+  }
+  s.cell = -1;
+  s.f0 = s.f1 = 0.0;
+}
+
 // ENDPOINT a5/O8 (SURVEY P-7): J_f = G(X1 - f) - G(X0 - f) for a particle that went from
-// (c0, xi0) to (c1, xi1) crossing k faces (signed).  With g0(x) = 1 - (1-x)^2/2 (own left
-// face) and g1(x) = x^2/2 (own right face):
-//   J_f = [faces passed completely: +-1] + g0(xi1)[f=c1] + g1(xi1)[f=c1+1]
-//                                       - g0(xi0)[f=c0] - g1(xi0)[f=c0+1].
+// (c0, x0) to (c1, x1) crossing k faces (signed).  With g0(x) = 1 - (1-x)^2/2 (own left face)
+// and g1(x) = x^2/2 (own right face):
+//   J_f = [faces passed completely: +-1] + g0(x1)[f=c1] + g1(x1)[f=c1+1]
+//                                       - g0(x0)[f=c0] - g1(x0)[f=c0+1].
 // The +-1 run covers faces [c0, c0+k) for k > 0 and [c1, c1+|k|) for k < 0 (periodic); it goes
 // into the difference array sD (prefix-summed at the block flush), whole turns of the ring into
-// sD[0].
+// sD[0].  Start-cell terms go through the lane's register accumulator.
 __device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_t* __restrict__ sD,
-                                                 int32_t n, int32_t c0, double x0, int32_t c1,
-                                                 double x1, int32_t k) {
-  const int32_t c0r = (c0 + 1 == n) ? 0 : c0 + 1;
-  const int32_t c1r = (c1 + 1 == n) ? 0 : c1 + 1;
+                                                 int32_t n, StartAcc& acc, int32_t c0, double x0,
+                                                 int32_t c1, double x1, int32_t k) {
+  if (c0 != acc.cell) {
+    flush_start(sF, n, acc);
+    acc.cell = c0;
+  }
   if (k == 0) {
-    // same cell: one term per face, no cancellation between atomics
+    // same cell: one term per face, no cancellation between large numbers
     const double d = x1 - x0, m = 0.5 * (x0 + x1);
-    atomicAdd(&sF[c0], d * (1.0 - m));
-    atomicAdd(&sF[c0r], d * m);
+    acc.f0 += d * (1.0 - m);
+    acc.f1 += d * m;
     return;
   }
+  acc.f0 += 0.5 * (1.0 - x0) * (1.0 - x0) - 1.0;
+  acc.f1 -= 0.5 * x0 * x0;
   atomicAdd(&sF[c1], 1.0 - 0.5 * (1.0 - x1) * (1.0 - x1));
-  atomicAdd(&sF[c1r], 0.5 * x1 * x1);
-  atomicAdd(&sF[c0], 0.5 * (1.0 - x0) * (1.0 - x0) - 1.0);
-  atomicAdd(&sF[c0r], -0.5 * x0 * x0);
+  atomicAdd(&sF[(c1 + 1 == n) ? 0 : c1 + 1], 0.5 * x1 * x1);
   const int32_t sgn = k > 0 ? 1 : -1;
   int32_t len = k > 0 ? k : -k;
   const int32_t a = k > 0 ? c0 : c1;
@@ -178,11 +205,19 @@ __device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_
   }
 }
 
-// One sub-step (O3-O8) of the lane's particle.  CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.
-template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT>
-__device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restrict__ sA,
-                                        double* __restrict__ sF, Lane<T>& p,
-                                        unsigned& picard_its, unsigned* diag) {
+// A-9: an orbit that reaches max_substeps with time left is parked with r < 0.
+template <typename T>
+__device__ __forceinline__ void count_substep(const MoverArgs<T>& a, Lane<T>& p) {
+  p.ns++;
+  if (p.ns >= (uint32_t)a.max_substeps && p.r > T(0)) p.r = -p.r;
+}
+
+// Tentative sub-step (O3-O6): estimate dtau, Crank-Nicolson step in the current cell; accept it
+// if it stays in the cell, otherwise leave a pending crossing in p.pdt.
+// CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.
+template <typename T, bool CN_DIRECT, bool DIAG>
+__device__ __forceinline__ void tentative(const MoverArgs<T>& a, Lane<T>& p,
+                                          unsigned& picard_its, unsigned* diag) {
   // ---- a2 / O4: estimator (Eq. 6-8), L1 form, in cell units:
   //   alpha = dx (|A| + |dA u|)/2, beta = eps_r dx (|A| + |u|)
   //   dtau = max( sqrt(eps_a/alpha), beta/alpha ) = max( c_abs d, c_rel (|A|+|u|) d^2 ),
@@ -196,8 +231,7 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
   if (DIAG && dtau > p.cap) diag[ST_KAPPA_CAP]++;
   dtau = tmin(tmin(dtau, p.cap), p.r);
 
-  // ---- a3 / O5: tentative Crank-Nicolson step over dtau with the linear field of the
-  // current cell (A-4).
+  // ---- a3 / O5: Crank-Nicolson step over dtau with the linear field of the current cell (A-4).
   T u1;
   if (CN_DIRECT) {
     // Eq. 11: kappa = a' dtau^2/4;  u' = [A dtau + (1+kappa) u] / (1-kappa).
@@ -229,44 +263,54 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     p.xi = xi1;
     p.u = u1;
     p.r -= dtau;
+    count_substep(a, p);
   } else {
-    // ---- a4 / O7: crossing.  Land on the face the tentative step left through.
-    const bool right = xi1 > T(1);
-    const T face = right ? T(1) : T(0);
-    const T dxi = face - p.xi;                        // signed distance to that face
-    const T Am = fma(T(0.5) * p.dA, dxi, A);          // A at the midpoint of the truncated step
-    T D = fma(T(2) * Am, dxi, p.u * p.u);             // Eq. 12 (energy principle)
-    if (DIAG && D < T(0)) diag[ST_NEG_DISC]++;
-    D = tmax(D, T(0));
-    const T sq = Prim<T>::sqrt(D);
-    const T uc = right ? sq : -sq;
-    // Root of F(dtau) = (A_m/2) dtau^2 + u dtau - dxi.  A-6: 2 dxi/(u+uc) when moving
-    // towards the face (the common case), Eq. 13 (uc-u)/A_m otherwise.
-    const bool toward = right ? (p.u > T(0)) : (p.u < T(0));
-    T dtc;
-    if (toward) {
-      dtc = Prim<T>::div(T(2) * dxi, p.u + uc);
-    } else {
-      dtc = (Am == T(0)) ? dtau : Prim<T>::div(uc - p.u, Am);
-    }
-    if (DIAG && !(dtc >= T(0) && dtc <= dtau)) diag[ST_CLAMPED]++;
-    dtc = tmin(tmax(dtc, T(0)), dtau);                // NaN -> 0 (IEEE max/min drop the NaN)
-    // a5: PER_VISIT flushes this cell visit now; ENDPOINT only counts the face.
-    if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, face);
-    else p.k += right ? 1 : -1;
-    // enter the neighbour on its near face
-    int32_t cn = right ? p.c + 1 : p.c - 1;
-    cn = (cn == a.n_cells) ? 0 : cn;
-    cn = (cn < 0) ? a.n_cells - 1 : cn;
-    p.c = cn;
-    p.xi = T(1) - face;
-    if (PER_VISIT) p.xa = p.xi;
-    p.u = uc;
-    p.r -= dtc;
-    p.nc++;
-    load_cell<T>(sA, a.c_cap, p);
+    p.pdt = (xi1 > T(1)) ? dtau : -dtau;
   }
-  p.ns++;
+}
+
+// a4 / O7: crossing of the pending tentative step: land on the face it left through.
+template <typename T, bool DIAG, bool PER_VISIT>
+__device__ __forceinline__ void cross(const MoverArgs<T>& a, const T* __restrict__ sA,
+                                      double* __restrict__ sF, Lane<T>& p, unsigned* diag) {
+  const bool right = p.pdt > T(0);
+  const T dtau = tabs(p.pdt);
+  const T face = right ? T(1) : T(0);
+  const T A = fma(p.dA, p.xi, p.AL);
+  const T dxi = face - p.xi;                        // signed distance to that face
+  const T Am = fma(T(0.5) * p.dA, dxi, A);          // A at the midpoint of the truncated step
+  T D = fma(T(2) * Am, dxi, p.u * p.u);             // Eq. 12 (energy principle)
+  if (DIAG && D < T(0)) diag[ST_NEG_DISC]++;
+  D = tmax(D, T(0));
+  const T sq = Prim<T>::sqrt(D);
+  const T uc = right ? sq : -sq;
+  // Root of F(dtau) = (A_m/2) dtau^2 + u dtau - dxi.  A-6: 2 dxi/(u+uc) when moving
+  // towards the face (the common case), Eq. 13 (uc-u)/A_m otherwise.
+  const bool toward = (right ? p.u : -p.u) > T(0);
+  T dtc;
+  if (toward) {
+    dtc = Prim<T>::div(T(2) * dxi, p.u + uc);
+  } else {
+    dtc = (Am == T(0)) ? dtau : Prim<T>::div(uc - p.u, Am);
+  }
+  if (DIAG && !(dtc >= T(0) && dtc <= dtau)) diag[ST_CLAMPED]++;
+  dtc = tmin(tmax(dtc, T(0)), dtau);                // NaN -> 0 (IEEE max/min drop the NaN)
+  // a5: PER_VISIT flushes this cell visit now; ENDPOINT only counts the face.
+  if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, face);
+  else p.k += right ? 1 : -1;
+  // enter the neighbour on its near face
+  int32_t cn = right ? p.c + 1 : p.c - 1;
+  cn = (cn == a.n_cells) ? 0 : cn;
+  cn = (cn < 0) ? a.n_cells - 1 : cn;
+  p.c = cn;
+  p.xi = T(1) - face;
+  if (PER_VISIT) p.xa = p.xi;
+  p.u = uc;
+  p.r -= dtc;
+  p.nc++;
+  p.pdt = T(0);
+  load_cell<T>(sA, a.c_cap, p);
+  count_substep(a, p);
 }
 
 template <typename T> struct LaunchCfg { static constexpr int min_blocks = 2; };
@@ -293,13 +337,16 @@ mover_kernel(const MoverArgs<T> a) {
 
   const int lane = threadIdx.x & 31;
   const unsigned lt_mask = (1u << lane) - 1u;
-  long long next = 0, end = 0;       // warp-uniform: the warp's current index range
+  const uint32_t n32 = (uint32_t)a.n;
+  uint32_t next = 0, end = 0;        // warp-uniform: the warp's current index range
   bool exhausted = false;            // the global queue has run dry
-  bool active = false;
   Lane<T> p;
-  p.idx = -1;
-  p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xa = T(0);
+  p.have = false;
+  p.idx = 0;
+  p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xa = p.pdt = T(0);
   p.c = p.k = p.c0 = 0; p.ns = p.nc = 0;
+  StartAcc acc;
+  acc.cell = -1; acc.f0 = acc.f1 = 0.0;
   unsigned long long tot_sub = 0, tot_cross = 0, tot_pic = 0;
   unsigned picard_its = 0;
   unsigned diag[ST_COUNT];
@@ -307,40 +354,48 @@ mover_kernel(const MoverArgs<T> a) {
   for (int i = 0; i < ST_COUNT; ++i) diag[i] = 0;
 
   for (;;) {
-    const unsigned parked = __ballot_sync(kFull, !active);
+    // ---- a6/a7/a1: lane-level re-queue.  Parked lanes (r <= 0) wait until enough of them have
+    // gathered, then store their result and pull the next particles of the warp's range.
+    const unsigned parked = __ballot_sync(kFull, !(p.r > T(0)));
     if (parked) {
       const int n_parked = __popc(parked);
       // steady state: refill once enough lanes are parked; tail (queue dry): wait for all 32.
       const bool go = exhausted ? (n_parked == 32) : (n_parked >= a.refill_threshold);
       if (go) {
         if (next >= end && !exhausted) {
-          // claim the next index range (a6: persistent-thread re-queue)
+          // claim the next index range (persistent-thread re-queue)
           unsigned long long t = 0;
           if (lane == 0) t = atomicAdd(a.queue, (unsigned long long)a.tile);
           t = __shfl_sync(kFull, t, 0);
-          if ((long long)t >= a.n) { exhausted = true; }
-          else { next = (long long)t; end = next + a.tile < a.n ? next + a.tile : a.n; }
+          if (t >= (unsigned long long)a.n) { exhausted = true; }
+          else {
+            next = (uint32_t)t;
+            end = (n32 - next > (uint32_t)a.tile) ? next + (uint32_t)a.tile : n32;
+          }
         }
-        if (!active) {
+        if (!(p.r > T(0))) {
           // ---- a7: store the parked result (state n+1) and deposit its current ...
-          if (p.idx >= 0) {
+          if (p.have) {
             if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, p.xi);
-            else deposit_endpoint(sF, sD, a.n_cells, p.c0, (double)p.xa, p.c, (double)p.xi, p.k);
+            else deposit_endpoint(sF, sD, a.n_cells, acc, p.c0, (double)p.xa, p.c, (double)p.xi, p.k);
             if (a.xi1) {
               a.xi1[p.idx] = p.xi;
               a.v1[p.idx] = p.u * a.dx;
               a.cell1[p.idx] = p.c;
             }
             if (a.nsub_out) { a.nsub_out[p.idx] = p.ns; a.ncross_out[p.idx] = p.nc; }
-            if (p.r > T(0)) diag[ST_SUBSTEP_CAP]++;        // cut off at max_substeps (A-9)
+            if (p.r < T(0)) diag[ST_SUBSTEP_CAP]++;        // cut off at max_substeps (A-9)
             tot_sub += p.ns; tot_cross += p.nc; tot_pic += picard_its;
             picard_its = 0;
-            p.idx = -1;
+            p.have = false;
+            p.r = T(0);
           }
           // ---- a1: ... and load the next particle of the range, if any.
-          const long long cand = next + __popc(parked & lt_mask);
-          if (cand < end) {
+          const uint32_t rank = (uint32_t)__popc(parked & lt_mask);
+          if (rank < end - next) {
+            const uint32_t cand = next + rank;
             p.idx = cand;
+            p.have = true;
             p.xi = a.xi0[cand];
             p.u = a.v0[cand] * a.inv_dx;
             p.c = a.cell0[cand];
@@ -350,18 +405,37 @@ mover_kernel(const MoverArgs<T> a) {
             p.k = 0;
             p.ns = 0; p.nc = 0;
             load_cell<T>(sA, a.c_cap, p);
-            active = p.r > T(0);
           }
         }
-        next = (next + n_parked < end) ? next + n_parked : end;
+        next = ((uint32_t)n_parked < end - next) ? next + (uint32_t)n_parked : end;
         if (exhausted && n_parked == 32) break;
       }
     }
-    if (active) {
-      substep<T, CN_DIRECT, DIAG, PER_VISIT>(a, sA, sF, p, picard_its, diag);
-      active = (p.r > T(0)) && (p.ns < (uint32_t)a.max_substeps);
+
+    // ---- sub-step rounds.  A lane steps unless it is parked or has a crossing pending; the
+    // crossing block runs once kCrossBatch lanes are pending (warp-level work compaction of the
+    // divergent branch).
+#pragma unroll
+    for (int j = 0; j < kInner; ++j) {
+      if (p.r > T(0) && p.pdt == T(0)) tentative<T, CN_DIRECT, DIAG>(a, p, picard_its, diag);
+      if (kCrossBatch <= 1) {
+        if (p.pdt != T(0)) cross<T, DIAG, PER_VISIT>(a, sA, sF, p, diag);
+      } else {
+        const unsigned pm = __ballot_sync(kFull, p.pdt != T(0));
+        if (__popc(pm) >= kCrossBatch) {
+          if (p.pdt != T(0)) cross<T, DIAG, PER_VISIT>(a, sA, sF, p, diag);
+        }
+      }
+    }
+    if (kCrossBatch > 1) {
+      // no lane left that can step: flush the pending crossings regardless of their number
+      const unsigned stepping = __ballot_sync(kFull, p.r > T(0) && p.pdt == T(0));
+      if (!stepping) {
+        if (p.pdt != T(0)) cross<T, DIAG, PER_VISIT>(a, sA, sF, p, diag);
+      }
     }
   }
+  if (!PER_VISIT) flush_start(sF, a.n_cells, acc);
 
   // ---- totals: warp reduce, one atomic per warp and slot.
 #pragma unroll
