@@ -146,6 +146,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1 << 22)
     ap.add_argument("--ref-sample", type=int, default=1 << 19)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: cell + velocity class)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -173,8 +174,9 @@ def main():
     sp = cfg["species"][0]
     n_p = sp["x"].shape[0]
     stream = torch.cuda.current_stream().cuda_stream
+    flags = 0 if args.no_vsort else B.PIC_FLAG_VSORT
     pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=args.precision,
-                cn_mode=args.cn_mode, stream=stream)
+                cn_mode=args.cn_mode, flags=flags, stream=stream)
     ng = cfg["n_cells"]
     dEn = torch.from_numpy(cfg["E_n"]).cuda()
     dEp = torch.from_numpy(cfg["E_np1"]).cuda()
@@ -263,6 +265,7 @@ def main():
         "dtype": "f32" if args.precision == "fp32" else "f64", "data": "synthetic",
         "config": {"workload": f"{args.workload}: {ng} cells, {n_p} particles/GPU, dt={dt}",
                    "precision": args.precision, "cn_mode": args.cn_mode,
+                   "binning": "cell" if args.no_vsort else "cell+velocity class (P:242-250)",
                    "substeps_per_particle": n_sub / max(n_p, 1),
                    "crossing_fraction": n_cross / max(n_sub, 1),
                    "l2": "inputs larger than L2 (particle state %.0f MB/GPU)" % (n_p * 12e-6),

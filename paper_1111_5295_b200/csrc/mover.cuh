@@ -104,9 +104,22 @@ template <> __device__ __forceinline__ double tmax<double>(double a, double b) {
 
 
 // Tuning constants of the warp scheduler inside the kernel.
-constexpr int kInner = 4;          // sub-step rounds between two refill votes
-constexpr int kCrossBatch = 1;     // pending crossings needed before the crossing block runs
-                                   // (1 = process at once)
+#ifndef PIC_KINNER
+#define PIC_KINNER 4
+#endif
+#ifndef PIC_KCROSS
+#define PIC_KCROSS 1
+#endif
+#ifndef PIC_REFILL
+#define PIC_REFILL 4
+#endif
+#ifndef PIC_MINBLOCKS_F32
+#define PIC_MINBLOCKS_F32 2
+#endif
+constexpr int kInner = PIC_KINNER;        // sub-step rounds between two refill votes
+constexpr int kCrossBatch = PIC_KCROSS;   // pending crossings needed before the crossing block
+                                          // runs (1 = process at once)
+constexpr int kRefill = PIC_REFILL;       // parked lanes needed before a refill
 
 // Per-lane particle registers.  r > 0 <=> an orbit is in flight; r < 0 marks an orbit cut off
 // at max_substeps (A-9).
@@ -314,6 +327,7 @@ __device__ __forceinline__ void cross(const MoverArgs<T>& a, const T* __restrict
 }
 
 template <typename T> struct LaunchCfg { static constexpr int min_blocks = 2; };
+template <> struct LaunchCfg<float> { static constexpr int min_blocks = PIC_MINBLOCKS_F32; };
 
 template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT>
 __global__ void __launch_bounds__(kBlock, LaunchCfg<T>::min_blocks)

@@ -58,20 +58,46 @@ int from_device(pic_handle* h, const double* dsrc, double* dst) {
   return PIC_OK;
 }
 
+VKey key_of(const SpeciesState& S) { return VKey{S.nv, S.vmean, S.vinv}; }
+
 template <typename T>
 int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double* dv_) {
   const int32_t ng = h->grid.n_cells;
   const double dx = h->grid.length / ng;
   const int b = h->cur;
-  // stage 1: cell/xi/v in input order into buffer 1-b, histogram
-  PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (ng + 1), h->stream));
+  S.nv = 1;
+  if (h->params.flags & PIC_FLAG_VSORT) {
+    // velocity classes: mean and sigma of the species' velocities (fp64 reduction, init only)
+    double* dm = nullptr;
+    double hm[2] = {0.0, 0.0};
+    PIC_CUDA(h, cudaMalloc(&dm, 2 * sizeof(double)));
+    cudaMemsetAsync(dm, 0, 2 * sizeof(double), h->stream);
+    moments_kernel<<<grid_for(S.n), 256, 0, h->stream>>>(S.n, dv_, dm);
+    cudaError_t e = cudaMemcpyAsync(hm, dm, sizeof hm, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(dm);
+    h->launches++;
+    if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "velocity moments", e);
+    const double mean = hm[0] / (double)S.n;
+    const double var = hm[1] / (double)S.n - mean * mean;
+    const long long nv = std::min<long long>(1024, h->n_keys / ng);
+    if (var > 0.0 && nv > 1) {
+      S.nv = (int32_t)nv;
+      S.vmean = mean;
+      S.vinv = (double)nv / (8.0 * std::sqrt(var));
+    }
+  }
+  const VKey vk = key_of(S);
+  const long long nk = (long long)ng * S.nv;
+  // stage 1: cell/xi/v in input order into buffer 1-b, histogram over the sort keys
+  PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (nk + 1), h->stream));
   bin_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, dx_, dv_, dx, h->grid.length, ng,
                                                       S.cell[1 - b], (T*)S.xi[1 - b],
-                                                      (T*)S.v[1 - b], h->d_hist, h->d_flag);
-  scan_kernel<<<1, 1024, 0, h->stream>>>(ng, h->d_hist);
+                                                      (T*)S.v[1 - b], h->d_hist, h->d_flag, vk);
+  scan_kernel<<<1, 1024, 0, h->stream>>>((int32_t)nk, h->d_hist);
   scatter_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(
       S.n, S.cell[1 - b], (const T*)S.xi[1 - b], (const T*)S.v[1 - b], nullptr, h->d_hist,
-      S.cell[b], (T*)S.xi[b], (T*)S.v[b], S.id[b]);
+      S.cell[b], (T*)S.xi[b], (T*)S.v[b], S.id[b], vk);
   h->launches += 3;
   PIC_CUDA(h, cudaGetLastError());
   return PIC_OK;
@@ -82,14 +108,17 @@ int rebin_species(pic_handle* h, SpeciesState& S) {
   // state n+1 lives in buffer 1-cur; scatter it, binned, into buffer cur (old state n is dead).
   const int32_t ng = h->grid.n_cells;
   const int src = 1 - h->cur, dst = h->cur;
-  PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (ng + 1), h->stream));
-  hist_kernel<<<grid_for(S.n), 256, 0, h->stream>>>(S.n, S.cell[src], h->d_hist);
-  scan_kernel<<<1, 1024, 0, h->stream>>>(ng, h->d_hist);
+  const VKey vk = key_of(S);
+  const long long nk = (long long)ng * S.nv;
+  PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (nk + 1), h->stream));
+  hist_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, S.cell[src], (const T*)S.v[src],
+                                                       h->d_hist, vk);
+  scan_kernel<<<1, 1024, 0, h->stream>>>((int32_t)nk, h->d_hist);
   // ids: buffer 1-cur was written in the order of buffer cur, so its ids are id[cur]; the
   // re-binned ids go to id[1-cur] and the two id arrays then trade places.
   scatter_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(
       S.n, S.cell[src], (const T*)S.xi[src], (const T*)S.v[src], S.id[dst], h->d_hist,
-      S.cell[dst], (T*)S.xi[dst], (T*)S.v[dst], S.id[src]);
+      S.cell[dst], (T*)S.xi[dst], (T*)S.v[dst], S.id[src], vk);
   std::swap(S.id[0], S.id[1]);
   h->launches += 3;
   PIC_CUDA(h, cudaGetLastError());
@@ -168,7 +197,11 @@ int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species,
   INIT_CUDA(cudaMalloc(&h->d_resid, sizeof(double) * ng));
   INIT_CUDA(cudaMalloc(&h->d_queue, sizeof(unsigned long long) * n_species));
   INIT_CUDA(cudaMalloc(&h->d_stats, sizeof(unsigned long long) * ST_COUNT));
-  INIT_CUDA(cudaMalloc(&h->d_hist, sizeof(int32_t) * (ng + 1)));
+  // sort keys: cells x velocity classes (<= 1024 classes, <= 4M keys)
+  h->n_keys = (params->flags & PIC_FLAG_VSORT)
+                  ? std::max<long long>(ng, std::min<long long>((long long)ng * 1024, 1LL << 22))
+                  : ng;
+  INIT_CUDA(cudaMalloc(&h->d_hist, sizeof(int32_t) * (h->n_keys + 1)));
   INIT_CUDA(cudaMalloc(&h->d_flag, sizeof(int32_t)));
   INIT_CUDA(cudaMemsetAsync(h->d_flag, 0, sizeof(int32_t), h->stream));
   INIT_CUDA(cudaEventCreate(&h->ev0));

@@ -20,6 +20,8 @@ struct SpeciesState {
   uint32_t* id[2] = {nullptr, nullptr};   // original index of the particle in each slot
   uint32_t* nsub = nullptr;               // optional per-particle counts of the last move
   uint32_t* ncross = nullptr;
+  int32_t nv = 1;                         // velocity classes of the sort key (1 = cell only)
+  double vmean = 0, vinv = 0;
   int grid_blocks = 0;                    // mover launch shape for this species
   int tile = 0;
 };
@@ -49,7 +51,8 @@ struct pic_handle {
   int total_rows = 0;
   unsigned long long* d_queue = nullptr;  // [n_species]
   unsigned long long* d_stats = nullptr;  // [ST_COUNT]
-  int32_t* d_hist = nullptr;              // [n_cells + 1] binning scratch
+  int32_t* d_hist = nullptr;              // [n_keys + 1] binning scratch
+  long long n_keys = 0;
   int32_t* d_flag = nullptr;              // validation flag
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   pic_stats stats{};

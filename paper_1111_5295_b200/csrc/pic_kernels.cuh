@@ -6,6 +6,44 @@
 
 namespace picb200 {
 
+// Sort key of the binning: cell only (nv = 1), or (cell, velocity class) with nv classes over
+// [vmean - 4 sigma, vmean + 4 sigma] (PIC_FLAG_VSORT; the paper's phase-space sort):
+// lanes of a warp then hold particles of one cell with similar velocities, whose sub-step and
+// crossing sequences are nearly the same.
+struct VKey {
+  int32_t nv;
+  double vmean, vinv;   // vinv = nv / (8 sigma)
+};
+__device__ __forceinline__ int32_t sort_key(const VKey& k, int32_t cell, double v) {
+  if (k.nv <= 1) return cell;
+  double t = (v - k.vmean) * k.vinv + 0.5 * k.nv;
+  int32_t b = (int32_t)fmin(fmax(t, 0.0), (double)(k.nv - 1));
+  return cell * k.nv + b;
+}
+
+// sum v, sum v^2 (fp64) -> out[0], out[1]
+static __global__ void moments_kernel(long long n, const double* __restrict__ v, double* __restrict__ out) {
+  __shared__ double r0[32], r1[32];
+  double s = 0.0, q = 0.0;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const double t = v[i];
+    s += t; q += t * t;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    s += __shfl_xor_sync(0xffffffffu, s, o);
+    q += __shfl_xor_sync(0xffffffffu, q, o);
+  }
+  if ((threadIdx.x & 31) == 0) { r0[threadIdx.x >> 5] = s; r1[threadIdx.x >> 5] = q; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { a += r0[w]; b += r1[w]; }
+    atomicAdd(&out[0], a);
+    atomicAdd(&out[1], b);
+  }
+}
+
 // x -> (cell, xi): cell = floor(x/dx) clipped to [0, n_cells-1], xi = x/dx - cell clipped to
 // [0,1] and rounded to T.  Also the per-cell histogram and input validation (flag != 0 if any
 // x is outside [0,L) or x / v is not finite).
@@ -13,7 +51,7 @@ template <typename T>
 __global__ void bin_kernel(long long n, const double* __restrict__ x, const double* __restrict__ v,
                            double dx, double length, int32_t n_cells, int32_t* __restrict__ cell,
                            T* __restrict__ xi, T* __restrict__ vout, int32_t* __restrict__ hist,
-                           int32_t* __restrict__ flag) {
+                           int32_t* __restrict__ flag, VKey vk) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x) {
     const double xv = x[i], vv = v[i];
@@ -28,17 +66,19 @@ __global__ void bin_kernel(long long n, const double* __restrict__ x, const doub
     cell[i] = c;
     xi[i] = (T)o;
     vout[i] = (T)vv;
-    atomicAdd(&hist[c], 1);
+    atomicAdd(&hist[sort_key(vk, c, (double)(T)vv)], 1);
   }
 }
 
-static __global__ void hist_kernel(long long n, const int32_t* __restrict__ cell, int32_t* __restrict__ hist) {
+template <typename T>
+__global__ void hist_kernel(long long n, const int32_t* __restrict__ cell, const T* __restrict__ v,
+                            int32_t* __restrict__ hist, VKey vk) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x)
-    atomicAdd(&hist[cell[i]], 1);
+    atomicAdd(&hist[sort_key(vk, cell[i], (double)v[i])], 1);
 }
 
-// Exclusive scan of hist[0..n_cells) in place (one block; n_cells is a few thousand at most).
+// Exclusive scan of hist[0..n_keys) in place (one block; at most a few million keys, init/commit only).
 static __global__ void scan_kernel(int32_t n_cells, int32_t* __restrict__ hist) {
   __shared__ int32_t carry;
   __shared__ int32_t wsum[32];
@@ -79,11 +119,11 @@ __global__ void scatter_kernel(long long n, const int32_t* __restrict__ cell_in,
                                const T* __restrict__ xi_in, const T* __restrict__ v_in,
                                const uint32_t* __restrict__ id_in, int32_t* __restrict__ cursor,
                                int32_t* __restrict__ cell_out, T* __restrict__ xi_out,
-                               T* __restrict__ v_out, uint32_t* __restrict__ id_out) {
+                               T* __restrict__ v_out, uint32_t* __restrict__ id_out, VKey vk) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x) {
     const int32_t c = cell_in[i];
-    const int32_t dst = atomicAdd(&cursor[c], 1);
+    const int32_t dst = atomicAdd(&cursor[sort_key(vk, c, (double)v_in[i])], 1);
     cell_out[dst] = c;
     xi_out[dst] = xi_in[i];
     v_out[dst] = v_in[i];

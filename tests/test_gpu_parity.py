@@ -85,6 +85,24 @@ def test_per_visit_deposit_parity(G, oracle, precision, which):
     g2["pic"].close()
 
 
+# ---- (cell, velocity class) binning: same results, original order kept ---------------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_vsort_parity_and_commit(G, oracle, precision):
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config2(n=150_001)
+    m = G.parity(oracle, cfg, precision, extra_flags=B.PIC_FLAG_VSORT)
+    _report(f"cfg2/150k {precision} vsort", m)
+    G.assert_parity(m, precision)
+    pic = m["gpu"]["pic"]
+    # commit re-bins by (cell, velocity class); getters still answer in the caller's order
+    before = pic.get_particles(0, B.PIC_STATE_NP1)
+    pic.commit()
+    after = pic.get_particles(0, B.PIC_STATE_N)
+    for k in ("x", "v", "cell", "xi"):
+        assert np.array_equal(before[k], after[k]), k
+    pic.close()
+
+
 # ---- long orbits: many wraps of the periodic ring (end-point deposit: whole turns) -----------
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_ring_wraps(G, oracle, precision):
