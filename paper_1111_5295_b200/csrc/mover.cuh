@@ -21,7 +21,9 @@
 //  * divergence (variable sub-step counts): persistent warps; a lane whose
 //    orbit is finished parks its result and, once enough lanes of the warp are parked, the
 //    parked lanes store and pull the next particles of the warp's current index range
-//    (lane-level re-queue); ranges are claimed from a global counter.
+//    (lane-level re-queue); ranges are claimed from a global counter.  With the state binned by
+//    (cell, velocity class) the lanes of a warp run nearly the same sub-step and
+//    crossing sequence, so both the crossing branch and the refill run with many lanes.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -52,6 +54,7 @@ struct MoverArgs {
   int32_t picard_max;
   int32_t tile;                // particles per claimed index range (multiple of 32)
   int32_t refill_threshold;    // parked lanes needed before a refill
+  int32_t wrap_mask;           // n_cells - 1 if n_cells is a power of two, else 0
   double qm_over_dx;           // (q/m)/dx
   T dx, inv_dx;
   T c_abs;                     // sqrt(2 eps_a / dx):   dtau_abs = c_abs / sqrt(|A| + |dA u|)
@@ -107,9 +110,6 @@ template <> __device__ __forceinline__ double tmax<double>(double a, double b) {
 #ifndef PIC_KINNER
 #define PIC_KINNER 4
 #endif
-#ifndef PIC_KCROSS
-#define PIC_KCROSS 1
-#endif
 #ifndef PIC_REFILL
 #define PIC_REFILL 4
 #endif
@@ -117,8 +117,6 @@ template <> __device__ __forceinline__ double tmax<double>(double a, double b) {
 #define PIC_MINBLOCKS_F32 2
 #endif
 constexpr int kInner = PIC_KINNER;        // sub-step rounds between two refill votes
-constexpr int kCrossBatch = PIC_KCROSS;   // pending crossings needed before the crossing block
-                                          // runs (1 = process at once)
 constexpr int kRefill = PIC_REFILL;       // parked lanes needed before a refill
 
 // Per-lane particle registers.  r > 0 <=> an orbit is in flight; r < 0 marks an orbit cut off
@@ -127,12 +125,10 @@ template <typename T>
 struct Lane {
   T xi, u, r;          // in-cell offset, velocity in cells/time, remaining time (O2)
   T AL, dA, cap;       // constants of the current cell (O3) and its kappa cap (A-2)
-  T pdt;               // pending crossing: +dtau (right face) / -dtau (left face); 0 = none
   T xa;                // ENDPOINT: xi at the orbit start;  PER_VISIT: xi at entry into the cell
   int32_t c;           // cell
-  int32_t k;           // ENDPOINT: signed number of faces crossed so far
   int32_t c0;          // ENDPOINT: start cell
-  uint32_t ns, nc;     // sub-steps, crossings of this orbit
+  uint32_t ns, nc, nr; // sub-steps, crossings, crossings through a right face (k = 2 nr - nc)
   uint32_t idx;        // particle index
   bool have;           // a particle (in flight or parked) occupies the lane
 };
@@ -218,19 +214,14 @@ __device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_
   }
 }
 
-// A-9: an orbit that reaches max_substeps with time left is parked with r < 0.
-template <typename T>
-__device__ __forceinline__ void count_substep(const MoverArgs<T>& a, Lane<T>& p) {
-  p.ns++;
-  if (p.ns >= (uint32_t)a.max_substeps && p.r > T(0)) p.r = -p.r;
-}
-
-// Tentative sub-step (O3-O6): estimate dtau, Crank-Nicolson step in the current cell; accept it
-// if it stays in the cell, otherwise leave a pending crossing in p.pdt.
-// CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.
-template <typename T, bool CN_DIRECT, bool DIAG>
-__device__ __forceinline__ void tentative(const MoverArgs<T>& a, Lane<T>& p,
-                                          unsigned& picard_its, unsigned* diag) {
+// One sub-step (O3-O8) of the lane's particle: estimate dtau, tentative Crank-Nicolson step in
+// the current cell, accept it if it stays in the cell, otherwise truncate it at the face.
+// CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.  The max_substeps cap (A-9) is checked by the
+// caller once every kInner sub-steps.
+template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT>
+__device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restrict__ sA,
+                                        double* __restrict__ sF, Lane<T>& p,
+                                        unsigned& picard_its, unsigned* diag) {
   // ---- a2 / O4: estimator (Eq. 6-8), L1 form, in cell units:
   //   alpha = dx (|A| + |dA u|)/2, beta = eps_r dx (|A| + |u|)
   //   dtau = max( sqrt(eps_a/alpha), beta/alpha ) = max( c_abs d, c_rel (|A|+|u|) d^2 ),
@@ -270,60 +261,54 @@ __device__ __forceinline__ void tentative(const MoverArgs<T>& a, Lane<T>& p,
     u1 = uk;
   }
   const T xi1 = fma(T(0.5) * dtau, p.u + u1, p.xi);   // Eq. 9
+  p.ns++;
 
   if (xi1 >= T(0) && xi1 <= T(1)) {
     // ---- O6: accept (inclusive, A-5).
     p.xi = xi1;
     p.u = u1;
     p.r -= dtau;
-    count_substep(a, p);
   } else {
-    p.pdt = (xi1 > T(1)) ? dtau : -dtau;
+    // ---- a4 / O7: crossing.  Land on the face the tentative step left through.
+    const bool right = xi1 > T(1);
+    const T face = right ? T(1) : T(0);
+    const T dxi = face - p.xi;                        // signed distance to that face
+    const T Am = fma(T(0.5) * p.dA, dxi, A);          // A at the midpoint of the truncated step
+    T D = fma(Am + Am, dxi, p.u * p.u);               // Eq. 12 (energy principle)
+    if (DIAG && D < T(0)) diag[ST_NEG_DISC]++;
+    D = tmax(D, T(0));
+    const T sq = Prim<T>::sqrt(D);
+    const T uc = right ? sq : -sq;
+    // Root of F(dtau) = (A_m/2) dtau^2 + u dtau - dxi.  A-6: 2 dxi/(u+uc) when moving
+    // towards the face (the common case), Eq. 13 (uc-u)/A_m otherwise.
+    const bool toward = (right ? p.u : -p.u) > T(0);
+    T dtc;
+    if (toward) {
+      dtc = Prim<T>::div(dxi + dxi, p.u + uc);
+    } else {
+      dtc = (Am == T(0)) ? dtau : Prim<T>::div(uc - p.u, Am);
+    }
+    if (DIAG && !(dtc >= T(0) && dtc <= dtau)) diag[ST_CLAMPED]++;
+    dtc = tmin(tmax(dtc, T(0)), dtau);                // NaN -> 0 (IEEE max/min drop the NaN)
+    // a5: PER_VISIT flushes this cell visit now; ENDPOINT only counts the face.
+    if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, face);
+    // enter the neighbour on its near face
+    int32_t cn = p.c + (right ? 1 : -1);
+    if (a.wrap_mask) {
+      cn &= a.wrap_mask;
+    } else {
+      cn = (cn == a.n_cells) ? 0 : cn;
+      cn = (cn < 0) ? a.n_cells - 1 : cn;
+    }
+    p.c = cn;
+    p.nc++;
+    if (right) p.nr++;
+    p.xi = T(1) - face;
+    if (PER_VISIT) p.xa = p.xi;
+    p.u = uc;
+    p.r -= dtc;
+    load_cell<T>(sA, a.c_cap, p);
   }
-}
-
-// a4 / O7: crossing of the pending tentative step: land on the face it left through.
-template <typename T, bool DIAG, bool PER_VISIT>
-__device__ __forceinline__ void cross(const MoverArgs<T>& a, const T* __restrict__ sA,
-                                      double* __restrict__ sF, Lane<T>& p, unsigned* diag) {
-  const bool right = p.pdt > T(0);
-  const T dtau = tabs(p.pdt);
-  const T face = right ? T(1) : T(0);
-  const T A = fma(p.dA, p.xi, p.AL);
-  const T dxi = face - p.xi;                        // signed distance to that face
-  const T Am = fma(T(0.5) * p.dA, dxi, A);          // A at the midpoint of the truncated step
-  T D = fma(T(2) * Am, dxi, p.u * p.u);             // Eq. 12 (energy principle)
-  if (DIAG && D < T(0)) diag[ST_NEG_DISC]++;
-  D = tmax(D, T(0));
-  const T sq = Prim<T>::sqrt(D);
-  const T uc = right ? sq : -sq;
-  // Root of F(dtau) = (A_m/2) dtau^2 + u dtau - dxi.  A-6: 2 dxi/(u+uc) when moving
-  // towards the face (the common case), Eq. 13 (uc-u)/A_m otherwise.
-  const bool toward = (right ? p.u : -p.u) > T(0);
-  T dtc;
-  if (toward) {
-    dtc = Prim<T>::div(T(2) * dxi, p.u + uc);
-  } else {
-    dtc = (Am == T(0)) ? dtau : Prim<T>::div(uc - p.u, Am);
-  }
-  if (DIAG && !(dtc >= T(0) && dtc <= dtau)) diag[ST_CLAMPED]++;
-  dtc = tmin(tmax(dtc, T(0)), dtau);                // NaN -> 0 (IEEE max/min drop the NaN)
-  // a5: PER_VISIT flushes this cell visit now; ENDPOINT only counts the face.
-  if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, face);
-  else p.k += right ? 1 : -1;
-  // enter the neighbour on its near face
-  int32_t cn = right ? p.c + 1 : p.c - 1;
-  cn = (cn == a.n_cells) ? 0 : cn;
-  cn = (cn < 0) ? a.n_cells - 1 : cn;
-  p.c = cn;
-  p.xi = T(1) - face;
-  if (PER_VISIT) p.xa = p.xi;
-  p.u = uc;
-  p.r -= dtc;
-  p.nc++;
-  p.pdt = T(0);
-  load_cell<T>(sA, a.c_cap, p);
-  count_substep(a, p);
 }
 
 template <typename T> struct LaunchCfg { static constexpr int min_blocks = 2; };
@@ -357,8 +342,8 @@ mover_kernel(const MoverArgs<T> a) {
   Lane<T> p;
   p.have = false;
   p.idx = 0;
-  p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xa = p.pdt = T(0);
-  p.c = p.k = p.c0 = 0; p.ns = p.nc = 0;
+  p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xa = T(0);
+  p.c = p.c0 = 0; p.ns = p.nc = p.nr = 0;
   StartAcc acc;
   acc.cell = -1; acc.f0 = acc.f1 = 0.0;
   unsigned long long tot_sub = 0, tot_cross = 0, tot_pic = 0;
@@ -368,6 +353,10 @@ mover_kernel(const MoverArgs<T> a) {
   for (int i = 0; i < ST_COUNT; ++i) diag[i] = 0;
 
   for (;;) {
+    // A-9: an orbit that has used max_substeps with time left is parked with r < 0 (checked
+    // once per kInner sub-steps, so it may overshoot the cap by fewer than kInner).
+    if (p.ns >= (uint32_t)a.max_substeps && p.r > T(0)) p.r = -p.r;
+
     // ---- a6/a7/a1: lane-level re-queue.  Parked lanes (r <= 0) wait until enough of them have
     // gathered, then store their result and pull the next particles of the warp's range.
     const unsigned parked = __ballot_sync(kFull, !(p.r > T(0)));
@@ -391,7 +380,8 @@ mover_kernel(const MoverArgs<T> a) {
           // ---- a7: store the parked result (state n+1) and deposit its current ...
           if (p.have) {
             if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, p.xi);
-            else deposit_endpoint(sF, sD, a.n_cells, acc, p.c0, (double)p.xa, p.c, (double)p.xi, p.k);
+            else deposit_endpoint(sF, sD, a.n_cells, acc, p.c0, (double)p.xa, p.c, (double)p.xi,
+                                  (int32_t)(2u * p.nr - p.nc));
             if (a.xi1) {
               a.xi1[p.idx] = p.xi;
               a.v1[p.idx] = p.u * a.dx;
@@ -403,6 +393,7 @@ mover_kernel(const MoverArgs<T> a) {
             picard_its = 0;
             p.have = false;
             p.r = T(0);
+            p.ns = 0;
           }
           // ---- a1: ... and load the next particle of the range, if any.
           const uint32_t rank = (uint32_t)__popc(parked & lt_mask);
@@ -416,8 +407,7 @@ mover_kernel(const MoverArgs<T> a) {
             p.r = a.dt;
             p.xa = p.xi;
             p.c0 = p.c;
-            p.k = 0;
-            p.ns = 0; p.nc = 0;
+            p.ns = 0; p.nc = 0; p.nr = 0;
             load_cell<T>(sA, a.c_cap, p);
           }
         }
@@ -426,27 +416,10 @@ mover_kernel(const MoverArgs<T> a) {
       }
     }
 
-    // ---- sub-step rounds.  A lane steps unless it is parked or has a crossing pending; the
-    // crossing block runs once kCrossBatch lanes are pending (warp-level work compaction of the
-    // divergent branch).
+    // ---- kInner sub-steps of every lane that has an orbit in flight
 #pragma unroll
     for (int j = 0; j < kInner; ++j) {
-      if (p.r > T(0) && p.pdt == T(0)) tentative<T, CN_DIRECT, DIAG>(a, p, picard_its, diag);
-      if (kCrossBatch <= 1) {
-        if (p.pdt != T(0)) cross<T, DIAG, PER_VISIT>(a, sA, sF, p, diag);
-      } else {
-        const unsigned pm = __ballot_sync(kFull, p.pdt != T(0));
-        if (__popc(pm) >= kCrossBatch) {
-          if (p.pdt != T(0)) cross<T, DIAG, PER_VISIT>(a, sA, sF, p, diag);
-        }
-      }
-    }
-    if (kCrossBatch > 1) {
-      // no lane left that can step: flush the pending crossings regardless of their number
-      const unsigned stepping = __ballot_sync(kFull, p.r > T(0) && p.pdt == T(0));
-      if (!stepping) {
-        if (p.pdt != T(0)) cross<T, DIAG, PER_VISIT>(a, sA, sF, p, diag);
-      }
+      if (p.r > T(0)) substep<T, CN_DIRECT, DIAG, PER_VISIT>(a, sA, sF, p, picard_its, diag);
     }
   }
   if (!PER_VISIT) flush_start(sF, a.n_cells, acc);
