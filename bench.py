@@ -170,7 +170,8 @@ def main():
     B.load()
 
     # replicas only: every rank runs its own copy of the workload with its own seed
-    cfg = _workload(args.workload, args.n, args.seed + rank)
+    from paper_1111_5295_b200 import replicas as _rep
+    cfg = _workload(args.workload, args.n, _rep.rank_seed(args.seed, rank))
     sp = cfg["species"][0]
     n_p = sp["x"].shape[0]
     stream = torch.cuda.current_stream().cuda_stream
@@ -226,16 +227,8 @@ def main():
         kms.append(pic.get_stats()["last_move_ms"])
     k_ms = float(np.mean(kms))
 
-    if world > 1:
-        t = torch.tensor([ms, e2e_s, float(n_sub), float(n_cross)], dtype=torch.float64, device="cuda")
-        tmax = t.clone()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone()
-        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms, e2e_s = float(tmax[0]), float(tmax[1])
-        tot_sub, tot_cross = float(tsum[2]), float(tsum[3])
-    else:
-        tot_sub, tot_cross = float(n_sub), float(n_cross)
+    from paper_1111_5295_b200 import replicas
+    ms, e2e_s, tot_sub, tot_cross = replicas.aggregate(ms, e2e_s, n_sub, n_cross, device="cuda")
     if rank != 0:
         pic.close()
         if world > 1:

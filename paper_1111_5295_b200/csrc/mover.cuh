@@ -108,16 +108,20 @@ template <> __device__ __forceinline__ double tmax<double>(double a, double b) {
 
 // Tuning constants of the warp scheduler inside the kernel.
 #ifndef PIC_KINNER
-#define PIC_KINNER 4
+#define PIC_KINNER 8
 #endif
 #ifndef PIC_REFILL
 #define PIC_REFILL 4
 #endif
+#ifndef PIC_REFILL_VSORT
+#define PIC_REFILL_VSORT 16
+#endif
 #ifndef PIC_MINBLOCKS_F32
-#define PIC_MINBLOCKS_F32 2
+#define PIC_MINBLOCKS_F32 3
 #endif
 constexpr int kInner = PIC_KINNER;        // sub-step rounds between two refill votes
-constexpr int kRefill = PIC_REFILL;       // parked lanes needed before a refill
+constexpr int kRefill = PIC_REFILL;       // parked lanes needed before a refill (cell binning)
+constexpr int kRefillVsort = PIC_REFILL_VSORT;  // same with (cell, velocity class) binning
 
 // Per-lane particle registers.  r > 0 <=> an orbit is in flight; r < 0 marks an orbit cut off
 // at max_substeps (A-9).
