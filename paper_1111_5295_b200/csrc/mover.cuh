@@ -108,13 +108,13 @@ template <> __device__ __forceinline__ double tmax<double>(double a, double b) {
 
 // Tuning constants of the warp scheduler inside the kernel.
 #ifndef PIC_KINNER
-#define PIC_KINNER 8
+#define PIC_KINNER 16
 #endif
 #ifndef PIC_REFILL
 #define PIC_REFILL 4
 #endif
 #ifndef PIC_REFILL_VSORT
-#define PIC_REFILL_VSORT 16
+#define PIC_REFILL_VSORT 24
 #endif
 #ifndef PIC_MINBLOCKS_F32
 #define PIC_MINBLOCKS_F32 3
