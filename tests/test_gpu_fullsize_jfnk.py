@@ -1,0 +1,110 @@
+"""`-m gpu`: (1) parity at BASELINE.json's full size (configs[2], 1e8 particles) in the launch
+configuration bench.py times: sampled orbits against the oracle one by one, plus the invariants
+that hold at any size (continuity, energy identity); (2) the host JFNK driver around the GPU
+mover (configs[1] shape, reduced particle count) checked with the oracle's residual."""
+import ctypes as C
+import math
+
+import numpy as np
+import pytest
+
+from paper_1111_5295_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _device_state(pic, B, torch, which):
+    n = pic.n[0]
+    cell = torch.empty(n, dtype=torch.int32, device="cuda")
+    xi = torch.empty(n, dtype=torch.float64, device="cuda")
+    v = torch.empty(n, dtype=torch.float64, device="cuda")
+    pic._chk(pic._L.pic_get_particles(pic._h, C.c_int(0), C.c_int(which), None, B._ptr(v),
+                                      B._ptr(cell), B._ptr(xi)))
+    return cell, xi, v
+
+
+def test_cfg2_full_size_sampled(oracle):
+    import torch
+    from paper_1111_5295_b200 import binding as B
+    import gpu_helpers as G
+    cfg = W.config2()                      # 4,096 cells, 1e8 electrons, dt = 10
+    sp = cfg["species"][0]
+    n, ng, dt = sp["x"].shape[0], cfg["n_cells"], cfg["dt"]
+    dx = cfg["length"] / ng
+    pic = B.Pic(ng, cfg["length"], [sp], precision="fp32", cn_mode="direct",
+                flags=B.PIC_FLAG_VSORT | B.PIC_FLAG_COUNTS,
+                stream=torch.cuda.current_stream().cuda_stream)
+    jbar = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], dt)
+    st = pic.get_stats()
+    assert st["n_substep_cap"] == 0 and st["n_sub"] > 40 * n
+    c0, x0, v0 = _device_state(pic, B, torch, B.PIC_STATE_N)
+    c1, x1, v1 = _device_state(pic, B, torch, B.PIC_STATE_NP1)
+    nsub = torch.empty(n, dtype=torch.int32, device="cuda")
+    ncross = torch.empty(n, dtype=torch.int32, device="cuda")
+    pic._chk(pic._L.pic_get_counts(pic._h, C.c_int(0), B._ptr(nsub), B._ptr(ncross)))
+    # ---- sampled orbits, one by one through the oracle (particles are independent given E)
+    idx = torch.from_numpy(np.sort(np.random.default_rng(3).choice(n, 1 << 16, replace=False))).cuda()
+    h = lambda t: t[idx].cpu().numpy()
+    r = oracle.move_accumulate(ng, cfg["length"], sp["q_over_m"], sp["w_q"], h(c0), h(x0) * dx,
+                               h(v0), cfg["E_n"], cfg["E_np1"], dt, oracle.make_params())
+    same = (r["n_sub"] == h(nsub).astype(np.uint32)) & (r["n_cross"] == h(ncross).astype(np.uint32)) \
+        & (r["cell"] == h(c1))
+    flips = int((~same).sum())
+    xg = (h(c1) + h(x1)) * dx
+    xr = r["cell"] * dx + r["s"]
+    ex = np.linalg.norm(G.periodic_dist(xg[same], xr[same], cfg["length"])) / np.linalg.norm(xr[same])
+    ev = G.rel_l2(h(v1)[same], r["v"][same])
+    print(f"[full] sampled 65536 of {n}: x={ex:.2e} v={ev:.2e} flips={flips}")
+    assert flips <= 1e-3 * idx.numel() and ex <= 1e-5 and ev <= 1e-5
+    # ---- energy identity (P-9) at full size
+    dK = pic.kinetic_energy(B.PIC_STATE_NP1)[0] - pic.kinetic_energy(B.PIC_STATE_N)[0]
+    work = dt * dx * np.sum(jbar * 0.5 * (cfg["E_n"] + cfg["E_np1"]))
+    print(f"[full] energy identity rel={(dK - work) / abs(work):.2e}")
+    assert abs(dK - work) <= 1e-4 * abs(work)
+    # ---- per-cell continuity (P-6) at full size, rho by the oracle in fp64 from the kernel's
+    # own (cell, xi)
+    rho0 = oracle.rho(ng, cfg["length"], sp["w_q"], c0.cpu().numpy(), x0.cpu().numpy() * dx)
+    rho1 = oracle.rho(ng, cfg["length"], sp["w_q"], c1.cpu().numpy(), x1.cpu().numpy() * dx)
+    div = dt * (np.roll(jbar, -1) - jbar) / dx
+    cont = np.linalg.norm(rho1 - rho0 + div) / np.linalg.norm(div)
+    print(f"[full] continuity rel={cont:.2e}")
+    assert cont <= 1e-5
+    # the device rho diagnostic agrees with the oracle's
+    assert G.rel_l2(pic.rho(B.PIC_STATE_NP1), rho1) < 1e-10
+    pic.close()
+
+
+def test_jfnk_steps_iaw(oracle):
+    from paper_1111_5295_b200 import binding as B
+    import gpu_helpers as G
+    cfg = W._iaw("iaw-test", 64, 500, 1.0, W.DEFAULT_SEED)     # configs[1] shape, 2 x 32,000
+    ng, L, dt = cfg["n_cells"], cfg["length"], cfg["dt"]
+    dx = L / ng
+    pic = B.Pic(ng, L, cfg["species"], precision="fp64", cn_mode="direct")
+    # A-13: E0 from the discrete Gauss law (E_{c+1} - E_c)/dx = rho_c, zero mean
+    rho = pic.rho(B.PIC_STATE_N)
+    E = np.concatenate(([0.0], np.cumsum(rho[:-1] * dx)))
+    E -= E.mean()
+
+    def energy():
+        return float(pic.kinetic_energy(B.PIC_STATE_N).sum() + 0.5 * dx * np.sum(E * E))
+
+    e0 = energy()
+    for step in range(3):
+        En = E.copy()
+        before = [pic.get_particles(j, B.PIC_STATE_N) for j in range(2)]
+        info = pic.jfnk_step(E, dt, rtol=1e-9)
+        assert info["rc"] == 0 and info["converged"] == 1, info
+        assert info["resid"] <= 1e-9 * info["resid0"] * 1.0001
+        # the oracle's residual at the converged field, from the same state n, is as small
+        state = [(b["cell"], b["xi"] * dx, b["v"]) for b in before]
+        c2 = dict(cfg, E_n=En, E_np1=E)
+        ref = G.oracle_run(oracle, c2, oracle.make_params(cn_mode=oracle.DIRECT), state=state)
+        R = oracle.residual(En, E, dt, ref["jbar"])
+        print(f"[jfnk] step {step}: newton={info['newton_its']} gmres={info['gmres_its']} "
+              f"|R0|={info['resid0']:.2e} |R|={info['resid']:.2e} oracle |R|={np.linalg.norm(R):.2e} "
+              f"dE/E={(energy() - e0) / e0:.2e}")
+        assert np.linalg.norm(R) <= 1e-7 * info["resid0"]
+    # energy conserved to the nonlinear tolerance level
+    assert abs(energy() - e0) / e0 < 1e-8
+    pic.close()
