@@ -108,7 +108,10 @@ template <> __device__ __forceinline__ double tmax<double>(double a, double b) {
 
 // Tuning constants of the warp scheduler inside the kernel.
 #ifndef PIC_KINNER
-#define PIC_KINNER 16
+#define PIC_KINNER 32
+#endif
+#ifndef PIC_UNROLL
+#define PIC_UNROLL 8
 #endif
 #ifndef PIC_REFILL
 #define PIC_REFILL 4
@@ -119,6 +122,7 @@ template <> __device__ __forceinline__ double tmax<double>(double a, double b) {
 #ifndef PIC_MINBLOCKS_F32
 #define PIC_MINBLOCKS_F32 3
 #endif
+constexpr int kUnroll = PIC_UNROLL;       // unroll factor of the sub-step rounds
 constexpr int kInner = PIC_KINNER;        // sub-step rounds between two refill votes
 constexpr int kRefill = PIC_REFILL;       // parked lanes needed before a refill (cell binning)
 constexpr int kRefillVsort = PIC_REFILL_VSORT;  // same with (cell, velocity class) binning
@@ -130,9 +134,10 @@ struct Lane {
   T xi, u, r;          // in-cell offset, velocity in cells/time, remaining time (O2)
   T AL, dA, cap;       // constants of the current cell (O3) and its kappa cap (A-2)
   T xa;                // ENDPOINT: xi at the orbit start;  PER_VISIT: xi at entry into the cell
-  int32_t c;           // cell
+  int32_t c;           // cell; with POW2 the UNWRAPPED cell c0 + k (wrapped by a mask on use)
   int32_t c0;          // ENDPOINT: start cell
-  uint32_t ns, nc, nr; // sub-steps, crossings, crossings through a right face (k = 2 nr - nc)
+  uint32_t ns, nc, nr; // sub-steps, crossings, crossings through a right face (k = 2 nr - nc;
+                       // nr is not kept with POW2, where k = c - c0)
   uint32_t idx;        // particle index
   bool have;           // a particle (in flight or parked) occupies the lane
 };
@@ -147,8 +152,8 @@ struct StartAcc {
 // O3: constants of cell c.  sA carries a one-face halo on both sides: sA[f+1] = A_f,
 // sA[0] = A_{n-1}, sA[n+1] = A_0, so the two faces of cell c are sA[c+1], sA[c+2].
 template <typename T>
-__device__ __forceinline__ void load_cell(const T* __restrict__ sA, T c_cap, Lane<T>& p) {
-  const T AL = sA[p.c + 1], AR = sA[p.c + 2];
+__device__ __forceinline__ void load_cell(const T* __restrict__ sA, T c_cap, Lane<T>& p, int32_t c) {
+  const T AL = sA[c + 1], AR = sA[c + 2];
   p.AL = AL;
   p.dA = AR - AL;
   // A-2: dtau <= sqrt(4 kappa_max / |a'|); |dA| = 0 gives +inf (no cap).
@@ -222,7 +227,7 @@ __device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_
 // the current cell, accept it if it stays in the cell, otherwise truncate it at the face.
 // CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.  The max_substeps cap (A-9) is checked by the
 // caller once every kInner sub-steps.
-template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT>
+template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2>
 __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restrict__ sA,
                                         double* __restrict__ sF, Lane<T>& p,
                                         unsigned& picard_its, unsigned* diag) {
@@ -295,30 +300,34 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     if (DIAG && !(dtc >= T(0) && dtc <= dtau)) diag[ST_CLAMPED]++;
     dtc = tmin(tmax(dtc, T(0)), dtau);                // NaN -> 0 (IEEE max/min drop the NaN)
     // a5: PER_VISIT flushes this cell visit now; ENDPOINT only counts the face.
-    if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, face);
     // enter the neighbour on its near face
-    int32_t cn = p.c + (right ? 1 : -1);
-    if (a.wrap_mask) {
-      cn &= a.wrap_mask;
+    int32_t cw;                                       // wrapped index of the new cell
+    if (POW2) {
+      if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c & a.wrap_mask, p.xa, face);
+      p.c += right ? 1 : -1;                          // unwrapped: k = c - c0
+      cw = p.c & a.wrap_mask;
     } else {
+      if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, face);
+      int32_t cn = p.c + (right ? 1 : -1);
       cn = (cn == a.n_cells) ? 0 : cn;
       cn = (cn < 0) ? a.n_cells - 1 : cn;
+      p.c = cn;
+      cw = cn;
+      if (right) p.nr++;
     }
-    p.c = cn;
     p.nc++;
-    if (right) p.nr++;
     p.xi = T(1) - face;
     if (PER_VISIT) p.xa = p.xi;
     p.u = uc;
     p.r -= dtc;
-    load_cell<T>(sA, a.c_cap, p);
+    load_cell<T>(sA, a.c_cap, p, cw);
   }
 }
 
 template <typename T> struct LaunchCfg { static constexpr int min_blocks = 2; };
 template <> struct LaunchCfg<float> { static constexpr int min_blocks = PIC_MINBLOCKS_F32; };
 
-template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT>
+template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2>
 __global__ void __launch_bounds__(kBlock, LaunchCfg<T>::min_blocks)
 mover_kernel(const MoverArgs<T> a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -383,9 +392,12 @@ mover_kernel(const MoverArgs<T> a) {
         if (!(p.r > T(0))) {
           // ---- a7: store the parked result (state n+1) and deposit its current ...
           if (p.have) {
-            if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, p.c, p.xa, p.xi);
-            else deposit_endpoint(sF, sD, a.n_cells, acc, p.c0, (double)p.xa, p.c, (double)p.xi,
-                                  (int32_t)(2u * p.nr - p.nc));
+            // canonical end cell and signed face count
+            const int32_t c1 = POW2 ? (p.c & a.wrap_mask) : p.c;
+            const int32_t k = POW2 ? (p.c - p.c0) : (int32_t)(2u * p.nr - p.nc);
+            if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, c1, p.xa, p.xi);
+            else deposit_endpoint(sF, sD, a.n_cells, acc, p.c0, (double)p.xa, c1, (double)p.xi, k);
+            p.c = c1;
             if (a.xi1) {
               a.xi1[p.idx] = p.xi;
               a.v1[p.idx] = p.u * a.dx;
@@ -412,7 +424,7 @@ mover_kernel(const MoverArgs<T> a) {
             p.xa = p.xi;
             p.c0 = p.c;
             p.ns = 0; p.nc = 0; p.nr = 0;
-            load_cell<T>(sA, a.c_cap, p);
+            load_cell<T>(sA, a.c_cap, p, p.c);
           }
         }
         next = ((uint32_t)n_parked < end - next) ? next + (uint32_t)n_parked : end;
@@ -421,9 +433,9 @@ mover_kernel(const MoverArgs<T> a) {
     }
 
     // ---- kInner sub-steps of every lane that has an orbit in flight
-#pragma unroll
+#pragma unroll kUnroll
     for (int j = 0; j < kInner; ++j) {
-      if (p.r > T(0)) substep<T, CN_DIRECT, DIAG, PER_VISIT>(a, sA, sF, p, picard_its, diag);
+      if (p.r > T(0)) substep<T, CN_DIRECT, DIAG, PER_VISIT, POW2>(a, sA, sF, p, picard_its, diag);
     }
   }
   if (!PER_VISIT) flush_start(sF, a.n_cells, acc);

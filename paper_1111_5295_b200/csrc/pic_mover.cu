@@ -10,27 +10,33 @@ namespace picb200 {
 
 namespace {
 
-// Dispatch over the kernel's template switches (CN mode, diagnostics, deposit mode).
-template <typename T, typename F>
-auto with_kernel(bool direct, bool diag, bool per_visit, F&& f) {
+// Dispatch over the kernel's template switches (CN mode, diagnostics, deposit mode, power-of-two
+// grid).
+template <typename T, bool P2, typename F>
+auto with_kernel_p(bool direct, bool diag, bool per_visit, F&& f) {
   const int key = (direct ? 4 : 0) | (diag ? 2 : 0) | (per_visit ? 1 : 0);
   switch (key) {
-    case 0: return f(mover_kernel<T, false, false, false>);
-    case 1: return f(mover_kernel<T, false, false, true>);
-    case 2: return f(mover_kernel<T, false, true, false>);
-    case 3: return f(mover_kernel<T, false, true, true>);
-    case 4: return f(mover_kernel<T, true, false, false>);
-    case 5: return f(mover_kernel<T, true, false, true>);
-    case 6: return f(mover_kernel<T, true, true, false>);
-    default: return f(mover_kernel<T, true, true, true>);
+    case 0: return f(mover_kernel<T, false, false, false, P2>);
+    case 1: return f(mover_kernel<T, false, false, true, P2>);
+    case 2: return f(mover_kernel<T, false, true, false, P2>);
+    case 3: return f(mover_kernel<T, false, true, true, P2>);
+    case 4: return f(mover_kernel<T, true, false, false, P2>);
+    case 5: return f(mover_kernel<T, true, false, true, P2>);
+    case 6: return f(mover_kernel<T, true, true, false, P2>);
+    default: return f(mover_kernel<T, true, true, true, P2>);
   }
+}
+template <typename T, typename F>
+auto with_kernel(bool direct, bool diag, bool per_visit, bool pow2, F&& f) {
+  return pow2 ? with_kernel_p<T, true>(direct, diag, per_visit, f)
+              : with_kernel_p<T, false>(direct, diag, per_visit, f);
 }
 
 template <typename T>
 cudaError_t set_smem_all(size_t bytes) {
   cudaError_t e = cudaSuccess;
-  for (int key = 0; key < 8 && e == cudaSuccess; ++key)
-    e = with_kernel<T>(key & 4, key & 2, key & 1, [&](auto k) {
+  for (int key = 0; key < 16 && e == cudaSuccess; ++key)
+    e = with_kernel<T>(key & 4, key & 2, key & 1, key & 8, [&](auto k) {
       return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     });
   return e;
@@ -39,7 +45,7 @@ cudaError_t set_smem_all(size_t bytes) {
 template <typename T>
 int occupancy(size_t bytes) {
   int nb = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, true, false, false>, kBlock, bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, true, false, false, true>, kBlock, bytes);
   return nb;
 }
 
@@ -88,7 +94,7 @@ void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const do
   const bool diag = (P.flags & PIC_FLAG_DIAG) != 0;
   const bool per_visit = (P.flags & PIC_FLAG_DEPOSIT_PER_VISIT) != 0;
   dim3 g(S.grid_blocks), b(kBlock);
-  with_kernel<T>(direct, diag, per_visit, [&](auto k) {
+  with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, [&](auto k) {
     k<<<g, b, h->smem_bytes, h->stream>>>(a);
     return cudaSuccess;
   });
