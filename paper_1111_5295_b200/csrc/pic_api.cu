@@ -58,13 +58,25 @@ int from_device(pic_handle* h, const double* dsrc, double* dst) {
   return PIC_OK;
 }
 
-VKey key_of(const SpeciesState& S) { return VKey{S.nv, S.vmean, S.vinv}; }
+VKey key_of(const SpeciesState& S) { return VKey{S.nx, S.nv, S.vmean, S.vinv}; }
+
+// exclusive scan of d_hist[0..nk) (three small kernels)
+int scan_hist(pic_handle* h, long long nk) {
+  const int chunks = (int)((nk + kScanChunk - 1) / kScanChunk);
+  scan_sums_kernel<<<chunks, kScanThreads, 0, h->stream>>>(nk, h->d_hist, h->d_scan);
+  scan_top_kernel<<<1, kScanThreads, 0, h->stream>>>(chunks, h->d_scan);
+  scan_chunks_kernel<<<chunks, kScanThreads, 0, h->stream>>>(nk, h->d_hist, h->d_scan);
+  h->launches += 3;
+  PIC_CUDA(h, cudaGetLastError());
+  return PIC_OK;
+}
 
 template <typename T>
 int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double* dv_) {
   const int32_t ng = h->grid.n_cells;
   const double dx = h->grid.length / ng;
   const int b = h->cur;
+  S.nx = 1;
   S.nv = 1;
   if (h->params.flags & PIC_FLAG_VSORT) {
     // velocity classes: mean and sigma of the species' velocities (fp64 reduction, init only)
@@ -80,25 +92,32 @@ int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double*
     if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "velocity moments", e);
     const double mean = hm[0] / (double)S.n;
     const double var = hm[1] / (double)S.n - mean * mean;
-    const long long nv = std::min<long long>(1024, h->n_keys / ng);
+    // classes: about 4 particles per phase-space cell, nx <= 8 offset classes, nv <= 1024
+    // velocity classes (powers of two), at most n_keys keys in all
+    const double ppc = (double)S.n / ng;
+    int32_t nx = 8, nv = 1;
+    while (nv < 1024 && (double)nx * nv * 2 * 4 <= ppc) nv *= 2;
+    while (nx > 1 && (long long)ng * nx * nv > h->n_keys) nx /= 2;
+    while (nv > 1 && (long long)ng * nx * nv > h->n_keys) nv /= 2;
     if (var > 0.0 && nv > 1) {
-      S.nv = (int32_t)nv;
+      S.nx = nx;
+      S.nv = nv;
       S.vmean = mean;
       S.vinv = (double)nv / (8.0 * std::sqrt(var));
     }
   }
   const VKey vk = key_of(S);
-  const long long nk = (long long)ng * S.nv;
+  const long long nk = (long long)ng * S.nx * S.nv;
   // stage 1: cell/xi/v in input order into buffer 1-b, histogram over the sort keys
   PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (nk + 1), h->stream));
   bin_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, dx_, dv_, dx, h->grid.length, ng,
                                                       S.cell[1 - b], (T*)S.xi[1 - b],
                                                       (T*)S.v[1 - b], h->d_hist, h->d_flag, vk);
-  scan_kernel<<<1, 1024, 0, h->stream>>>((int32_t)nk, h->d_hist);
+  if (int rc = scan_hist(h, nk)) return rc;
   scatter_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(
       S.n, S.cell[1 - b], (const T*)S.xi[1 - b], (const T*)S.v[1 - b], nullptr, h->d_hist,
       S.cell[b], (T*)S.xi[b], (T*)S.v[b], S.id[b], vk);
-  h->launches += 3;
+  h->launches += 2;
   PIC_CUDA(h, cudaGetLastError());
   return PIC_OK;
 }
@@ -109,18 +128,18 @@ int rebin_species(pic_handle* h, SpeciesState& S) {
   const int32_t ng = h->grid.n_cells;
   const int src = 1 - h->cur, dst = h->cur;
   const VKey vk = key_of(S);
-  const long long nk = (long long)ng * S.nv;
+  const long long nk = (long long)ng * S.nx * S.nv;
   PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (nk + 1), h->stream));
-  hist_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, S.cell[src], (const T*)S.v[src],
-                                                       h->d_hist, vk);
-  scan_kernel<<<1, 1024, 0, h->stream>>>((int32_t)nk, h->d_hist);
+  hist_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, S.cell[src], (const T*)S.xi[src],
+                                                       (const T*)S.v[src], h->d_hist, vk);
+  if (int rc = scan_hist(h, nk)) return rc;
   // ids: buffer 1-cur was written in the order of buffer cur, so its ids are id[cur]; the
   // re-binned ids go to id[1-cur] and the two id arrays then trade places.
   scatter_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(
       S.n, S.cell[src], (const T*)S.xi[src], (const T*)S.v[src], S.id[dst], h->d_hist,
       S.cell[dst], (T*)S.xi[dst], (T*)S.v[dst], S.id[src], vk);
   std::swap(S.id[0], S.id[1]);
-  h->launches += 3;
+  h->launches += 2;
   PIC_CUDA(h, cudaGetLastError());
   return PIC_OK;
 }
@@ -134,7 +153,7 @@ void free_all(pic_handle* h) {
   }
   cudaFree(h->dE_n); cudaFree(h->dE_step); cudaFree(h->dE_np1); cudaFree(h->d_jbar);
   cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue); cudaFree(h->d_stats);
-  cudaFree(h->d_hist); cudaFree(h->d_flag);
+  cudaFree(h->d_hist); cudaFree(h->d_flag); cudaFree(h->d_scan);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
 }
@@ -197,11 +216,12 @@ int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species,
   INIT_CUDA(cudaMalloc(&h->d_resid, sizeof(double) * ng));
   INIT_CUDA(cudaMalloc(&h->d_queue, sizeof(unsigned long long) * n_species));
   INIT_CUDA(cudaMalloc(&h->d_stats, sizeof(unsigned long long) * ST_COUNT));
-  // sort keys: cells x velocity classes (<= 1024 classes, <= 4M keys)
+  // sort keys: cells x offset classes x velocity classes, at most 2^24 keys (64 MB of counters)
   h->n_keys = (params->flags & PIC_FLAG_VSORT)
-                  ? std::max<long long>(ng, std::min<long long>((long long)ng * 1024, 1LL << 22))
+                  ? std::max<long long>(ng, std::min<long long>((long long)ng * 8192, 1LL << 24))
                   : ng;
   INIT_CUDA(cudaMalloc(&h->d_hist, sizeof(int32_t) * (h->n_keys + 1)));
+  INIT_CUDA(cudaMalloc(&h->d_scan, sizeof(int32_t) * (h->n_keys / kScanChunk + 2)));
   INIT_CUDA(cudaMalloc(&h->d_flag, sizeof(int32_t)));
   INIT_CUDA(cudaMemsetAsync(h->d_flag, 0, sizeof(int32_t), h->stream));
   INIT_CUDA(cudaEventCreate(&h->ev0));

@@ -20,7 +20,7 @@ struct SpeciesState {
   uint32_t* id[2] = {nullptr, nullptr};   // original index of the particle in each slot
   uint32_t* nsub = nullptr;               // optional per-particle counts of the last move
   uint32_t* ncross = nullptr;
-  int32_t nv = 1;                         // velocity classes of the sort key (1 = cell only)
+  int32_t nx = 1, nv = 1;                 // offset / velocity classes of the sort key (1 = cell only)
   double vmean = 0, vinv = 0;
   int grid_blocks = 0;                    // mover launch shape for this species
   int tile = 0;
@@ -53,6 +53,7 @@ struct pic_handle {
   unsigned long long* d_stats = nullptr;  // [ST_COUNT]
   int32_t* d_hist = nullptr;              // [n_keys + 1] binning scratch
   long long n_keys = 0;
+  int32_t* d_scan = nullptr;              // [n_keys / 4096 + 1] chunk sums of the scan
   int32_t* d_flag = nullptr;              // validation flag
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   pic_stats stats{};

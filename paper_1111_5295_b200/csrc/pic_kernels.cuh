@@ -6,19 +6,22 @@
 
 namespace picb200 {
 
-// Sort key of the binning: cell only (nv = 1), or (cell, velocity class) with nv classes over
-// [vmean - 4 sigma, vmean + 4 sigma] (PIC_FLAG_VSORT; the paper's phase-space sort):
-// lanes of a warp then hold particles of one cell with similar velocities, whose sub-step and
-// crossing sequences are nearly the same.
+// Sort key of the binning: cell only (nx = nv = 1), or with PIC_FLAG_VSORT the phase-space cell
+// (cell, xi class, velocity class) -- the paper's phase-space sort: nx classes of
+// the in-cell offset and nv velocity classes over [vmean - 4 sigma, vmean + 4 sigma], ordered so
+// that neighbours in memory share the cell and the offset class and have adjacent velocities.
+// Lanes of a warp then start almost the same orbit: same sub-step sequence, crossings in the same
+// round, orbit ends in the same round.
 struct VKey {
-  int32_t nv;
+  int32_t nx, nv;
   double vmean, vinv;   // vinv = nv / (8 sigma)
 };
-__device__ __forceinline__ int32_t sort_key(const VKey& k, int32_t cell, double v) {
-  if (k.nv <= 1) return cell;
-  double t = (v - k.vmean) * k.vinv + 0.5 * k.nv;
-  int32_t b = (int32_t)fmin(fmax(t, 0.0), (double)(k.nv - 1));
-  return cell * k.nv + b;
+__device__ __forceinline__ int32_t sort_key(const VKey& k, int32_t cell, double xi, double v) {
+  if (k.nv <= 1 && k.nx <= 1) return cell;
+  const double t = (v - k.vmean) * k.vinv + 0.5 * k.nv;
+  const int32_t b = (int32_t)fmin(fmax(t, 0.0), (double)(k.nv - 1));
+  const int32_t xb = min((int32_t)(xi * k.nx), k.nx - 1);
+  return (cell * k.nx + xb) * k.nv + b;
 }
 
 // sum v, sum v^2 (fp64) -> out[0], out[1]
@@ -66,49 +69,101 @@ __global__ void bin_kernel(long long n, const double* __restrict__ x, const doub
     cell[i] = c;
     xi[i] = (T)o;
     vout[i] = (T)vv;
-    atomicAdd(&hist[sort_key(vk, c, (double)(T)vv)], 1);
+    atomicAdd(&hist[sort_key(vk, c, (double)(T)o, (double)(T)vv)], 1);
   }
 }
 
 template <typename T>
-__global__ void hist_kernel(long long n, const int32_t* __restrict__ cell, const T* __restrict__ v,
-                            int32_t* __restrict__ hist, VKey vk) {
+__global__ void hist_kernel(long long n, const int32_t* __restrict__ cell, const T* __restrict__ xi,
+                            const T* __restrict__ v, int32_t* __restrict__ hist, VKey vk) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x)
-    atomicAdd(&hist[sort_key(vk, cell[i], (double)v[i])], 1);
+    atomicAdd(&hist[sort_key(vk, cell[i], (double)xi[i], (double)v[i])], 1);
 }
 
-// Exclusive scan of hist[0..n_keys) in place (one block; at most a few million keys, init/commit only).
-static __global__ void scan_kernel(int32_t n_cells, int32_t* __restrict__ hist) {
-  __shared__ int32_t carry;
+// Exclusive scan of hist[0..n) in place, three passes: per-chunk sums, scan of the chunk sums
+// (one block), per-chunk exclusive scan + offset.  kScanChunk elements per block.
+constexpr int kScanChunk = 4096;
+constexpr int kScanThreads = 512;
+
+static __device__ __forceinline__ int32_t block_exclusive_scan(int32_t val, int32_t* wsum, int32_t& total) {
+  // exclusive scan of one value per thread over a kScanThreads block
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int32_t inc = val;
+  for (int o = 1; o < 32; o <<= 1) {
+    const int32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) wsum[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    int32_t s = lane < (int)(blockDim.x >> 5) ? wsum[lane] : 0;
+    for (int o = 1; o < 32; o <<= 1) {
+      const int32_t t = __shfl_up_sync(0xffffffffu, s, o);
+      if (lane >= o) s += t;
+    }
+    wsum[lane] = s;   // inclusive over warps
+  }
+  __syncthreads();
+  total = wsum[(blockDim.x >> 5) - 1];
+  const int32_t r = (w ? wsum[w - 1] : 0) + inc - val;
+  __syncthreads();
+  return r;
+}
+
+static __global__ void scan_sums_kernel(long long n, const int32_t* __restrict__ hist,
+                                        int32_t* __restrict__ sums) {
+  __shared__ int32_t red[32];
+  const long long base = (long long)blockIdx.x * kScanChunk;
+  int32_t s = 0;
+  for (int i = threadIdx.x; i < kScanChunk; i += blockDim.x)
+    if (base + i < n) s += hist[base + i];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int32_t t = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
+    sums[blockIdx.x] = t;
+  }
+}
+
+// one block: exclusive scan of sums[0..m) in place (m = number of chunks, any size)
+static __global__ void scan_top_kernel(int32_t m, int32_t* __restrict__ sums) {
   __shared__ int32_t wsum[32];
+  __shared__ int32_t carry;
   if (threadIdx.x == 0) carry = 0;
   __syncthreads();
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  for (int base = 0; base < n_cells; base += blockDim.x) {
+  for (int base = 0; base < m; base += blockDim.x) {
     const int i = base + threadIdx.x;
-    const int32_t val = i < n_cells ? hist[i] : 0;
-    int32_t inc = val;
-    for (int o = 1; o < 32; o <<= 1) {
-      const int32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += t;
-    }
-    if (lane == 31) wsum[w] = inc;
+    const int32_t val = i < m ? sums[i] : 0;
+    int32_t total;
+    const int32_t ex = block_exclusive_scan(val, wsum, total);
+    if (i < m) sums[i] = carry + ex;
     __syncthreads();
-    if (w == 0) {
-      int32_t s = lane < (int)(blockDim.x >> 5) ? wsum[lane] : 0;
-      for (int o = 1; o < 32; o <<= 1) {
-        const int32_t t = __shfl_up_sync(0xffffffffu, s, o);
-        if (lane >= o) s += t;
-      }
-      wsum[lane] = s;   // inclusive over warps
-    }
+    if (threadIdx.x == 0) carry += total;
     __syncthreads();
-    const int32_t woff = w ? wsum[w - 1] : 0;
-    if (i < n_cells) hist[i] = carry + woff + inc - val;
-    __syncthreads();
-    if (threadIdx.x == 0) carry += wsum[(blockDim.x >> 5) - 1];
-    __syncthreads();
+  }
+}
+
+static __global__ void scan_chunks_kernel(long long n, int32_t* __restrict__ hist,
+                                          const int32_t* __restrict__ sums) {
+  __shared__ int32_t wsum[32];
+  constexpr int per = kScanChunk / kScanThreads;
+  const long long base = (long long)blockIdx.x * kScanChunk + (long long)threadIdx.x * per;
+  int32_t v[per];
+  int32_t s = 0;
+#pragma unroll
+  for (int j = 0; j < per; ++j) {
+    v[j] = (base + j < n) ? hist[base + j] : 0;
+    s += v[j];
+  }
+  int32_t total;
+  int32_t run = sums[blockIdx.x] + block_exclusive_scan(s, wsum, total);
+#pragma unroll
+  for (int j = 0; j < per; ++j) {
+    if (base + j < n) hist[base + j] = run;
+    run += v[j];
   }
 }
 
@@ -123,7 +178,7 @@ __global__ void scatter_kernel(long long n, const int32_t* __restrict__ cell_in,
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x) {
     const int32_t c = cell_in[i];
-    const int32_t dst = atomicAdd(&cursor[sort_key(vk, c, (double)v_in[i])], 1);
+    const int32_t dst = atomicAdd(&cursor[sort_key(vk, c, (double)xi_in[i], (double)v_in[i])], 1);
     cell_out[dst] = c;
     xi_out[dst] = xi_in[i];
     v_out[dst] = v_in[i];

@@ -75,7 +75,7 @@ void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const do
   a.wrap_mask = (h->grid.n_cells > 1 && (h->grid.n_cells & (h->grid.n_cells - 1)) == 0)
                     ? h->grid.n_cells - 1 : 0;
   // velocity-sorted warps finish in bunches: wait for a larger bunch before the refill block
-  a.refill_threshold = (S.nv > 1) ? kRefillVsort : kRefill;
+  a.refill_threshold = (S.nv > 1 || S.nx > 1) ? kRefillVsort : kRefill;
   a.qm_over_dx = S.q_over_m / dx;
   a.dx = (T)dx;
   a.inv_dx = (T)(1.0 / dx);
