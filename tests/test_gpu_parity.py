@@ -215,10 +215,11 @@ def test_substep_cap_is_reported(G):
     cfg = W.config2(n=2000)
     sp = cfg["species"][0]
     pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp64", max_substeps=4)
+    jbar = np.empty(cfg["n_cells"])            # must outlive the call: the library writes into it
     with pytest.raises(B.PicError) as ei:
         pic._chk(pic._L.pic_move_accumulate(pic._h, B._ptr(cfg["E_n"]), B._ptr(cfg["E_np1"]),
                                             B.C.c_double(cfg["dt"]), B.C.c_double(1e-10),
-                                            B._ptr(np.empty(cfg["n_cells"]))))
+                                            B._ptr(jbar)))
     assert ei.value.code == B.PIC_ERR_SUBSTEP_CAP
     assert pic.get_stats()["n_substep_cap"] > 0
     pic.close()
