@@ -146,7 +146,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1 << 22)
     ap.add_argument("--ref-sample", type=int, default=1 << 19)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: cell + velocity class)")
+    ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: phase-space cell)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -258,7 +258,7 @@ def main():
         "dtype": "f32" if args.precision == "fp32" else "f64", "data": "synthetic",
         "config": {"workload": f"{args.workload}: {ng} cells, {n_p} particles/GPU, dt={dt}",
                    "precision": args.precision, "cn_mode": args.cn_mode,
-                   "binning": "cell" if args.no_vsort else "cell+velocity class (P:242-250)",
+                   "binning": "cell" if args.no_vsort else "phase-space cell: cell + offset class + velocity class (P:242-250)",
                    "substeps_per_particle": n_sub / max(n_p, 1),
                    "crossing_fraction": n_cross / max(n_sub, 1),
                    "l2": "inputs larger than L2 (particle state %.0f MB/GPU)" % (n_p * 12e-6),

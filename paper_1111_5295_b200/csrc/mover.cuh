@@ -30,7 +30,10 @@
 
 namespace picb200 {
 
-constexpr int kBlock = 512;        // threads per block
+#ifndef PIC_BLOCK
+#define PIC_BLOCK 384
+#endif
+constexpr int kBlock = PIC_BLOCK;  // threads per block
 constexpr unsigned kFull = 0xffffffffu;
 
 enum StatSlot { ST_SUB = 0, ST_CROSS, ST_PICARD_IT, ST_PICARD_CAP, ST_KAPPA_CAP, ST_SUBSTEP_CAP,
@@ -189,9 +192,17 @@ __device__ __forceinline__ void flush_start(double* __restrict__ sF, int32_t n, 
 // The +-1 run covers faces [c0, c0+k) for k > 0 and [c1, c1+|k|) for k < 0 (periodic); it goes
 // into the difference array sD (prefix-summed at the block flush), whole turns of the ring into
 // sD[0].  Start-cell terms go through the lane's register accumulator.
+// End-cell terms are handed back (e0 on face c1, e1 on face c1+1; `pending` set) so that the warp
+// can add up the lanes that end in the same cell before touching shared memory.
+struct EndTerms {
+  double e0, e1;
+  int32_t cell;
+  bool pending;
+};
+
 __device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_t* __restrict__ sD,
-                                                 int32_t n, StartAcc& acc, int32_t c0, double x0,
-                                                 int32_t c1, double x1, int32_t k) {
+                                                 int32_t n, StartAcc& acc, EndTerms& et, int32_t c0,
+                                                 double x0, int32_t c1, double x1, int32_t k) {
   if (c0 != acc.cell) {
     flush_start(sF, n, acc);
     acc.cell = c0;
@@ -205,8 +216,10 @@ __device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_
   }
   acc.f0 += 0.5 * (1.0 - x0) * (1.0 - x0) - 1.0;
   acc.f1 -= 0.5 * x0 * x0;
-  atomicAdd(&sF[c1], 1.0 - 0.5 * (1.0 - x1) * (1.0 - x1));
-  atomicAdd(&sF[(c1 + 1 == n) ? 0 : c1 + 1], 0.5 * x1 * x1);
+  et.e0 = 1.0 - 0.5 * (1.0 - x1) * (1.0 - x1);
+  et.e1 = 0.5 * x1 * x1;
+  et.cell = c1;
+  et.pending = true;
   const int32_t sgn = k > 0 ? 1 : -1;
   int32_t len = k > 0 ? k : -k;
   const int32_t a = k > 0 ? c0 : c1;
@@ -220,6 +233,41 @@ __device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_
     atomicAdd(&sD[a], sgn);
     if (e < n) atomicAdd(&sD[e], -sgn);
     else if (e > n) { atomicAdd(&sD[0], sgn); atomicAdd(&sD[e - n], -sgn); }
+  }
+}
+
+// Warp-uniform: add the pending end-cell terms of all lanes to the block accumulators, one pair
+// of shared-memory atomics per DISTINCT end cell (lanes of a warp mostly end in the same one or
+// two cells, and the fp64 shared atomic is a CAS loop that would serialise them).
+__device__ __forceinline__ void warp_deposit_end(double* __restrict__ sF, int32_t n, int lane,
+                                                 const EndTerms& et) {
+  unsigned todo = __ballot_sync(kFull, et.pending);
+  bool mine_left = et.pending;
+  // up to two shared end cells are summed across the warp ...
+#pragma unroll 1
+  for (int it = 0; it < 2 && todo; ++it) {
+    const int leader = __ffs(todo) - 1;
+    const int32_t key = __shfl_sync(kFull, et.cell, leader);
+    const bool mine = mine_left && et.cell == key;
+    const unsigned grp = __ballot_sync(kFull, mine);
+    todo &= ~grp;
+    if (__popc(grp) == 1) continue;              // a singleton goes the direct way below
+    double a = mine ? et.e0 : 0.0, b = mine ? et.e1 : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      a += __shfl_xor_sync(kFull, a, o);
+      b += __shfl_xor_sync(kFull, b, o);
+    }
+    if (lane == leader) {
+      atomicAdd(&sF[key], a);
+      atomicAdd(&sF[(key + 1 == n) ? 0 : key + 1], b);
+    }
+    if (mine) mine_left = false;
+  }
+  // ... lanes that end anywhere else (long, scattered orbits) add their own terms
+  if (mine_left) {
+    atomicAdd(&sF[et.cell], et.e0);
+    atomicAdd(&sF[(et.cell + 1 == n) ? 0 : et.cell + 1], et.e1);
   }
 }
 
@@ -389,6 +437,8 @@ mover_kernel(const MoverArgs<T> a) {
             end = (n32 - next > (uint32_t)a.tile) ? next + (uint32_t)a.tile : n32;
           }
         }
+        EndTerms et;
+        et.pending = false; et.cell = 0; et.e0 = et.e1 = 0.0;
         if (!(p.r > T(0))) {
           // ---- a7: store the parked result (state n+1) and deposit its current ...
           if (p.have) {
@@ -396,7 +446,7 @@ mover_kernel(const MoverArgs<T> a) {
             const int32_t c1 = POW2 ? (p.c & a.wrap_mask) : p.c;
             const int32_t k = POW2 ? (p.c - p.c0) : (int32_t)(2u * p.nr - p.nc);
             if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, c1, p.xa, p.xi);
-            else deposit_endpoint(sF, sD, a.n_cells, acc, p.c0, (double)p.xa, c1, (double)p.xi, k);
+            else deposit_endpoint(sF, sD, a.n_cells, acc, et, p.c0, (double)p.xa, c1, (double)p.xi, k);
             p.c = c1;
             if (a.xi1) {
               a.xi1[p.idx] = p.xi;
@@ -427,6 +477,7 @@ mover_kernel(const MoverArgs<T> a) {
             load_cell<T>(sA, a.c_cap, p, p.c);
           }
         }
+        if (!PER_VISIT) warp_deposit_end(sF, a.n_cells, lane, et);
         next = ((uint32_t)n_parked < end - next) ? next + (uint32_t)n_parked : end;
         if (exhausted && n_parked == 32) break;
       }

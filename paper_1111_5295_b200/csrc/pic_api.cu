@@ -95,8 +95,14 @@ int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double*
     // classes: about 4 particles per phase-space cell, nx <= 8 offset classes, nv <= 1024
     // velocity classes (powers of two), at most n_keys keys in all
     const double ppc = (double)S.n / ng;
-    int32_t nx = 8, nv = 1;
-    while (nv < 1024 && (double)nx * nv * 2 * 4 <= ppc) nv *= 2;
+#ifndef PIC_NX
+#define PIC_NX 8
+#endif
+#ifndef PIC_PPK
+#define PIC_PPK 4
+#endif
+    int32_t nx = PIC_NX, nv = 1;
+    while (nv < 1024 && (double)nx * nv * 2 * PIC_PPK <= ppc) nv *= 2;
     while (nx > 1 && (long long)ng * nx * nv > h->n_keys) nx /= 2;
     while (nv > 1 && (long long)ng * nx * nv > h->n_keys) nv /= 2;
     if (var > 0.0 && nv > 1) {
