@@ -111,27 +111,26 @@ template <> __device__ __forceinline__ double tmax<double>(double a, double b) {
 
 // Tuning constants of the warp scheduler inside the kernel.
 #ifndef PIC_KINNER
-#define PIC_KINNER 32
+#define PIC_KINNER 64
 #endif
 #ifndef PIC_UNROLL
-#define PIC_UNROLL 8
+#define PIC_UNROLL 4
 #endif
 #ifndef PIC_REFILL
 #define PIC_REFILL 4
 #endif
 #ifndef PIC_REFILL_VSORT
-#define PIC_REFILL_VSORT 24
+#define PIC_REFILL_VSORT 28
 #endif
 #ifndef PIC_MINBLOCKS_F32
 #define PIC_MINBLOCKS_F32 3
 #endif
-constexpr int kUnroll = PIC_UNROLL;       // unroll factor of the sub-step rounds
+constexpr int kGroup = PIC_UNROLL;        // sub-steps between two "any lane still in flight" votes
 constexpr int kInner = PIC_KINNER;        // sub-step rounds between two refill votes
 constexpr int kRefill = PIC_REFILL;       // parked lanes needed before a refill (cell binning)
 constexpr int kRefillVsort = PIC_REFILL_VSORT;  // same with (cell, velocity class) binning
 
-// Per-lane particle registers.  r > 0 <=> an orbit is in flight; r < 0 marks an orbit cut off
-// at max_substeps (A-9).
+// Per-lane particle registers.  r > 0 <=> an orbit is in flight.
 template <typename T>
 struct Lane {
   T xi, u, r;          // in-cell offset, velocity in cells/time, remaining time (O2)
@@ -142,7 +141,8 @@ struct Lane {
   uint32_t ns, nc, nr; // sub-steps, crossings, crossings through a right face (k = 2 nr - nc;
                        // nr is not kept with POW2, where k = c - c0)
   uint32_t idx;        // particle index
-  bool have;           // a particle (in flight or parked) occupies the lane
+  int32_t have;        // 0 = lane empty, 1 = a particle (in flight or parked), 2 = parked
+                       // because it was cut off at max_substeps (A-9)
 };
 
 // ENDPOINT: start-cell terms are collected in registers while consecutive particles of the lane
@@ -318,7 +318,7 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     u1 = uk;
   }
   const T xi1 = fma(T(0.5) * dtau, p.u + u1, p.xi);   // Eq. 9
-  p.ns++;
+  if (p.r > T(0)) p.ns++;   // a parked lane (r = 0) takes a zero-length step that changes nothing
 
   if (xi1 >= T(0) && xi1 <= T(1)) {
     // ---- O6: accept (inclusive, A-5).
@@ -401,7 +401,7 @@ mover_kernel(const MoverArgs<T> a) {
   uint32_t next = 0, end = 0;        // warp-uniform: the warp's current index range
   bool exhausted = false;            // the global queue has run dry
   Lane<T> p;
-  p.have = false;
+  p.have = 0;
   p.idx = 0;
   p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xa = T(0);
   p.c = p.c0 = 0; p.ns = p.nc = p.nr = 0;
@@ -416,7 +416,7 @@ mover_kernel(const MoverArgs<T> a) {
   for (;;) {
     // A-9: an orbit that has used max_substeps with time left is parked with r < 0 (checked
     // once per kInner sub-steps, so it may overshoot the cap by fewer than kInner).
-    if (p.ns >= (uint32_t)a.max_substeps && p.r > T(0)) p.r = -p.r;
+    if (p.ns >= (uint32_t)a.max_substeps && p.r > T(0)) { p.r = T(0); p.have = 2; }
 
     // ---- a6/a7/a1: lane-level re-queue.  Parked lanes (r <= 0) wait until enough of them have
     // gathered, then store their result and pull the next particles of the warp's range.
@@ -454,10 +454,10 @@ mover_kernel(const MoverArgs<T> a) {
               a.cell1[p.idx] = p.c;
             }
             if (a.nsub_out) { a.nsub_out[p.idx] = p.ns; a.ncross_out[p.idx] = p.nc; }
-            if (p.r < T(0)) diag[ST_SUBSTEP_CAP]++;        // cut off at max_substeps (A-9)
+            if (p.have == 2) diag[ST_SUBSTEP_CAP]++;       // cut off at max_substeps (A-9)
             tot_sub += p.ns; tot_cross += p.nc; tot_pic += picard_its;
             picard_its = 0;
-            p.have = false;
+            p.have = 0;
             p.r = T(0);
             p.ns = 0;
           }
@@ -466,7 +466,7 @@ mover_kernel(const MoverArgs<T> a) {
           if (rank < end - next) {
             const uint32_t cand = next + rank;
             p.idx = cand;
-            p.have = true;
+            p.have = 1;
             p.xi = a.xi0[cand];
             p.u = a.v0[cand] * a.inv_dx;
             p.c = a.cell0[cand];
@@ -484,9 +484,15 @@ mover_kernel(const MoverArgs<T> a) {
     }
 
     // ---- kInner sub-steps of every lane that has an orbit in flight
-#pragma unroll kUnroll
-    for (int j = 0; j < kInner; ++j) {
-      if (p.r > T(0)) substep<T, CN_DIRECT, DIAG, PER_VISIT, POW2>(a, sA, sF, p, picard_its, diag);
+    // Every lane steps: with r = 0 (parked or empty) dtau = 0, the tentative step reproduces
+    // (xi, u) bit for bit and is accepted, so no per-lane guard branch is needed; the warp leaves
+    // the rounds early once no lane has an orbit in flight (checked every kGroup sub-steps).
+#pragma unroll 1
+    for (int j = 0; j < kInner / kGroup; ++j) {
+#pragma unroll
+      for (int g = 0; g < kGroup; ++g)
+        substep<T, CN_DIRECT, DIAG, PER_VISIT, POW2>(a, sA, sF, p, picard_its, diag);
+      if (!__any_sync(kFull, p.r > T(0))) break;
     }
   }
   if (!PER_VISIT) flush_start(sF, a.n_cells, acc);

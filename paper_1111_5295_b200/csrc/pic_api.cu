@@ -102,7 +102,10 @@ int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double*
 #define PIC_PPK 4
 #endif
     int32_t nx = PIC_NX, nv = 1;
-    while (nv < 1024 && (double)nx * nv * 2 * PIC_PPK <= ppc) nv *= 2;
+#ifndef PIC_NVMAX
+#define PIC_NVMAX 1024
+#endif
+    while (nv < PIC_NVMAX && (double)nx * nv * 2 * PIC_PPK <= ppc) nv *= 2;
     while (nx > 1 && (long long)ng * nx * nv > h->n_keys) nx /= 2;
     while (nv > 1 && (long long)ng * nx * nv > h->n_keys) nv /= 2;
     if (var > 0.0 && nv > 1) {
@@ -222,9 +225,12 @@ int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species,
   INIT_CUDA(cudaMalloc(&h->d_resid, sizeof(double) * ng));
   INIT_CUDA(cudaMalloc(&h->d_queue, sizeof(unsigned long long) * n_species));
   INIT_CUDA(cudaMalloc(&h->d_stats, sizeof(unsigned long long) * ST_COUNT));
+#ifndef PIC_KEYCAP_LOG2
+#define PIC_KEYCAP_LOG2 24
+#endif
   // sort keys: cells x offset classes x velocity classes, at most 2^24 keys (64 MB of counters)
   h->n_keys = (params->flags & PIC_FLAG_VSORT)
-                  ? std::max<long long>(ng, std::min<long long>((long long)ng * 8192, 1LL << 24))
+                  ? std::max<long long>(ng, std::min<long long>((long long)ng * 65536, 1LL << PIC_KEYCAP_LOG2))
                   : ng;
   INIT_CUDA(cudaMalloc(&h->d_hist, sizeof(int32_t) * (h->n_keys + 1)));
   INIT_CUDA(cudaMalloc(&h->d_scan, sizeof(int32_t) * (h->n_keys / kScanChunk + 2)));

@@ -210,11 +210,11 @@ def test_empty_species_and_bad_input(G):
 
 def test_substep_cap_is_reported(G):
     from paper_1111_5295_b200 import binding as B
-    # the kernel tests the cap once per 32 sub-steps (A-9), so take orbits that need
-    # more than that: configs[2] shape, ~47 sub-steps per particle
-    cfg = W.config2(n=2000)
+    # the kernel tests the cap once per 64 sub-steps (A-9), so take orbits that need
+    # many more than that: configs[3] shape, ~590 sub-steps per particle
+    cfg = W.config3(n=2000)
     sp = cfg["species"][0]
-    pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp64", max_substeps=4)
+    pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp64", max_substeps=16)
     jbar = np.empty(cfg["n_cells"])            # must outlive the call: the library writes into it
     with pytest.raises(B.PicError) as ei:
         pic._chk(pic._L.pic_move_accumulate(pic._h, B._ptr(cfg["E_n"]), B._ptr(cfg["E_np1"]),
