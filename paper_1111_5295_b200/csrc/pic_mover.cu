@@ -124,7 +124,10 @@ int mover_configure(pic_handle* h) {
     S.grid_blocks = (int)std::max<long long>(1, std::min(full, want));
     const long long warps = (long long)S.grid_blocks * (kBlock / 32);
     long long tile = S.n / (warps * 8);                 // >= 8 claims per warp
-    tile = std::max<long long>(32, std::min<long long>(1024, tile / 32 * 32));
+#ifndef PIC_TILE_MAX
+#define PIC_TILE_MAX 512
+#endif
+    tile = std::max<long long>(32, std::min<long long>(PIC_TILE_MAX, tile / 32 * 32));
     S.tile = (int)tile;
     rows += S.grid_blocks;
   }
