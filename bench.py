@@ -33,6 +33,9 @@ UNIT = "sub-steps/s"
 # Algorithmic op table (paper's convention: every FP / int / SF thread-operation = 1, FMA = 2;
 # P:94-105), SURVEY 8(d) / DESIGN.md 6: per in-cell sub-step and per crossing sub-step.
 OPS_INCELL, OPS_CROSS = 43.0, 72.0
+# dram__bytes_read.sum + dram__bytes_write.sum of one mover launch from the committed
+# `ncu --set full` capture (profiles/r1_mover_ncu.md); known only for the default workload.
+NCU_TRAFFIC_BYTES = {("cfg2", 100_000_000, "fp32"): 2.369e9}
 
 
 def _workload(name, n, seed):
@@ -269,7 +272,10 @@ def main():
                 "d2h_bytes_per_step": ng * 8},
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_gops, "unit": "GOp/s",
-                     "frac": achieved / peak_gops, "traffic": None,
+                     "frac": achieved / peak_gops,
+                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, n_p, args.precision)),
+                     "traffic_unit": "bytes per launch (ncu dram read+write); algorithmic %d"
+                                     % (n_p * (24 if args.precision == "fp32" else 40)),
                      "kernel": "mover_kernel", "kernel_ms": k_ms,
                      "ops_per_launch": ops_per_launch,
                      "peak_source": "derived: SMs x lanes x 2 x sm_max_mhz (DESIGN.md 6)",
