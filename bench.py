@@ -195,6 +195,14 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- one step of the counting build (PIC_FLAG_DIAG) for the exact sub-step / crossing
+    # counts of a step (state n is constant, so every step does the same work); the timed steps
+    # run the fast build, which does not count per sub-step
+    pic.set_flags(flags | B.PIC_FLAG_DIAG)
+    pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+    exact = pic.get_stats()
+    pic.set_flags(flags)
+
     # ---- device-resident timing
     for _ in range(args.warmup):
         pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
@@ -212,7 +220,8 @@ def main():
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
     st1 = pic.get_stats()
-    n_sub, n_cross = st1["n_sub"], st1["n_cross"]        # per step (state n is constant)
+    n_sub, n_cross = exact["n_sub"], exact["n_cross"]    # per step, exact
+    assert st1["n_cross"] == n_cross and n_sub <= st1["n_sub"] < n_sub + 4 * n_p
     launches = st1["n_launches"] - st0["n_launches"]
 
     # ---- end to end: host E^n, E^{n+1} in, host jbar out, every step

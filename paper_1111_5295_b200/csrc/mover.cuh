@@ -318,7 +318,9 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     u1 = uk;
   }
   const T xi1 = fma(T(0.5) * dtau, p.u + u1, p.xi);   // Eq. 9
-  if (p.r > T(0)) p.ns++;   // a parked lane (r = 0) takes a zero-length step that changes nothing
+  // exact per-particle sub-step count only in the counting build (DIAG); a parked lane (r = 0)
+  // takes a zero-length step that changes nothing and is not counted
+  if (DIAG) { if (p.r > T(0)) p.ns++; }
 
   if (xi1 >= T(0) && xi1 <= T(1)) {
     // ---- O6: accept (inclusive, A-5).
@@ -489,6 +491,9 @@ mover_kernel(const MoverArgs<T> a) {
     // the rounds early once no lane has an orbit in flight (checked every kGroup sub-steps).
 #pragma unroll 1
     for (int j = 0; j < kInner / kGroup; ++j) {
+      // fast build: sub-steps are counted per group of kGroup rounds (an upper bound, less than
+      // kGroup above the exact count per particle); it feeds the A-9 cap and pic_stats.n_sub
+      if (!DIAG) { if (p.r > T(0)) p.ns += kGroup; }
 #pragma unroll
       for (int g = 0; g < kGroup; ++g)
         substep<T, CN_DIRECT, DIAG, PER_VISIT, POW2>(a, sA, sF, p, picard_its, diag);

@@ -91,7 +91,8 @@ void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const do
   a.queue = h->d_queue + s;
   a.stats = h->d_stats;
   const bool direct = P.cn_mode == PIC_CN_DIRECT;
-  const bool diag = (P.flags & PIC_FLAG_DIAG) != 0;
+  // the counting build: exact per-particle sub-step counts and anomaly counters
+  const bool diag = (P.flags & (PIC_FLAG_DIAG | PIC_FLAG_COUNTS)) != 0;
   const bool per_visit = (P.flags & PIC_FLAG_DEPOSIT_PER_VISIT) != 0;
   dim3 g(S.grid_blocks), b(kBlock);
   with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, [&](auto k) {

@@ -103,6 +103,26 @@ def test_vsort_parity_and_commit(G, oracle, precision):
     pic.close()
 
 
+# ---- the fast build (no per-sub-step counting) computes the same orbits as the counting build --
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_fast_build_matches_counting_build(G, precision):
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config2(n=120_007)
+    sp = cfg["species"][0]
+    out = {}
+    for name, flags in (("fast", B.PIC_FLAG_VSORT), ("count", B.PIC_FLAG_VSORT | B.PIC_FLAG_DIAG)):
+        pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=precision, flags=flags)
+        j = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+        out[name] = (pic.get_particles(0, B.PIC_STATE_NP1), j, pic.get_stats())
+        pic.close()
+    (pf, jf, sf), (pc, jc, sc) = out["fast"], out["count"]
+    for k in ("x", "v", "cell", "xi"):
+        assert np.array_equal(pf[k], pc[k]), k            # bit-identical orbits
+    assert G.rel_l2(jf, jc) < 1e-13                       # same deposits, atomics in any order
+    assert sf["n_cross"] == sc["n_cross"]
+    assert sc["n_sub"] <= sf["n_sub"] < sc["n_sub"] + 4 * 120_007   # grouped upper bound
+
+
 # ---- long orbits: many wraps of the periodic ring (end-point deposit: whole turns) -----------
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_ring_wraps(G, oracle, precision):
