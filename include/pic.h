@@ -81,7 +81,8 @@ typedef struct pic_stats { /* totals of the LAST pic_move_accumulate over all sp
   int64_t n_sub;           /* sub-steps (in-cell + crossing): exact with PIC_FLAG_COUNTS or
                               PIC_FLAG_DIAG; without them the kernel counts in groups of 4
                               rounds and n_sub is an upper bound, < 4 per particle above       */
-  int64_t n_cross;         /* crossing sub-steps                                               */
+  int64_t n_cross;         /* crossing sub-steps: exact with PIC_FLAG_COUNTS or PIC_FLAG_DIAG;
+                              without them 0 on power-of-two grids (not counted)             */
   int64_t n_picard_it;     /* Picard iterations (PICARD mode)                                  */
   int64_t n_picard_cap;    /* sub-steps whose Picard loop hit picard_max      (DIAG)           */
   int64_t n_kappa_cap;     /* sub-steps limited by the kappa cap              (DIAG)           */

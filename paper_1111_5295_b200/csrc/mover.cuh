@@ -365,7 +365,9 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
       cw = cn;
       if (right) p.nr++;
     }
-    p.nc++;
+    // crossings are counted per particle where something needs them: the counting build, and
+    // k = 2 nr - nc of a non-power-of-two grid
+    if (DIAG || !POW2) p.nc++;
     p.xi = T(1) - face;
     if (PER_VISIT) p.xa = p.xi;
     p.u = uc;
