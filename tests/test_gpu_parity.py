@@ -123,6 +123,30 @@ def test_fast_build_matches_counting_build(G, precision):
     assert sc["n_sub"] <= sf["n_sub"] < sc["n_sub"] + 4 * 120_007   # grouped upper bound
 
 
+# ---- grids whose cell count is not a power of two take the generic wrap path --------------------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("n_cells", [3, 48, 100])
+def test_non_power_of_two_grid(G, oracle, precision, n_cells):
+    from paper_1111_5295_b200 import binding as B
+    length = 0.7 * n_cells
+    xf = W.face_positions(n_cells, length)
+    n = 30_011
+    x = W.uniform01(21, 1, n) * length * (1 - 1e-12)
+    v = 1.5 * W.normal01(21, 2, n)
+    cfg = dict(n_cells=n_cells, length=length, dt=4.0, tol=1e-12,
+               E_n=0.2 * np.sin(2 * math.pi * xf / length),
+               E_np1=0.2 * np.sin(2 * math.pi * xf / length + 0.4),
+               species=[dict(name="e", q_over_m=-1.0, w_q=-length / n, x=x, v=v)])
+    for extra in (0, B.PIC_FLAG_VSORT, B.PIC_FLAG_DEPOSIT_PER_VISIT):
+        m = G.parity(oracle, cfg, precision, extra_flags=extra)
+        _report(f"n_cells={n_cells} {precision} flags+{extra}", m)
+        G.assert_parity(m, precision, max_flip_frac=2e-3)
+        r = m["ref"]["species"][0]
+        unwrapped = r["cell0"].astype(np.int64) + r["k"]
+        assert np.any(unwrapped < 0) and np.any(unwrapped >= n_cells)     # orbits cross the seam
+        m["gpu"]["pic"].close()
+
+
 # ---- long orbits: many wraps of the periodic ring (end-point deposit: whole turns) -----------
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_ring_wraps(G, oracle, precision):
