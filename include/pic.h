@@ -173,14 +173,29 @@ typedef struct pic_jfnk_opts {
 typedef struct pic_jfnk_info {
   int32_t newton_its;
   int32_t gmres_its;
-  int32_t mover_calls;
+  int32_t mover_calls;     /* all mover calls of the step                                      */
   int32_t converged;
   double resid0;           /* ||R(E^n)||_2                                                     */
   double resid;            /* final ||R||_2                                                    */
+  int32_t mover_calls_resid; /* of which calls of the residual handle (all, without defect corr.) */
+  int32_t pad_;
 } pic_jfnk_info;
 
 int pic_jfnk_step(pic_handle* h, double* E, double dt, double tol, const pic_jfnk_opts* opts,
                   pic_jfnk_info* info);
+
+/* pic_jfnk_step_dc -- the same step with defect correction (S8(f) #2): the nonlinear
+ * residual comes from h_resid (the fp64 mover), the Jacobian-vector products of GMRES from h_jac
+ * (the fp32 mover, built from the SAME particles), so the converged E^{n+1} has the accuracy of
+ * the fp64 mover while most mover calls run in fp32.  On convergence h_resid is committed and
+ * h_jac takes over its state (pic_copy_state). */
+int pic_jfnk_step_dc(pic_handle* h_resid, pic_handle* h_jac, double* E, double dt, double tol,
+                     const pic_jfnk_opts* opts, pic_jfnk_info* info);
+
+/* pic_copy_state -- make state n of dst a copy of state n of src (same grid, same species and
+ * particle counts; precisions may differ: values are converted).  Binning order and original
+ * indices are carried over. */
+int pic_copy_state(pic_handle* dst, pic_handle* src);
 
 int pic_destroy(pic_handle* h);
 const char* pic_last_error(const pic_handle* h);

@@ -24,8 +24,8 @@ PIC_ERR_SUBSTEP_CAP = -4
 
 EXPORTS = ["pic_init", "pic_move_accumulate", "pic_set_step", "pic_residual", "pic_commit",
            "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_set_flags",
-           "pic_kinetic_energy", "pic_rho", "pic_jfnk_step", "pic_destroy", "pic_last_error",
-           "pic_version"]
+           "pic_kinetic_energy", "pic_rho", "pic_jfnk_step", "pic_jfnk_step_dc",
+           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_version"]
 
 
 class PicGrid(C.Structure):
@@ -62,7 +62,8 @@ class PicJfnkOpts(C.Structure):
 class PicJfnkInfo(C.Structure):
     _fields_ = [("newton_its", C.c_int32), ("gmres_its", C.c_int32),
                 ("mover_calls", C.c_int32), ("converged", C.c_int32),
-                ("resid0", C.c_double), ("resid", C.c_double)]
+                ("resid0", C.c_double), ("resid", C.c_double),
+                ("mover_calls_resid", C.c_int32), ("pad_", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -228,14 +229,24 @@ class Pic:
         self._chk(self._L.pic_rho(self._h, C.c_int(which), _ptr(out)))
         return out
 
+    def copy_state_from(self, other):
+        """pic_copy_state(self, other): state n of `other` becomes state n of this handle."""
+        self._chk(self._L.pic_copy_state(self._h, other._h))
+
     def jfnk_step(self, E, dt, tol=1e-10, rtol=1e-8, atol=0.0, fd_eps=0.0, gmres_rtol=1e-2,
-                  max_newton=20, gmres_restart=30, max_gmres=200):
-        """pic_jfnk_step: E (numpy float64[n_cells]) is E^n on entry, E^{n+1} on return."""
+                  max_newton=20, gmres_restart=30, max_gmres=200, jacobian=None):
+        """pic_jfnk_step: E (numpy float64[n_cells]) is E^n on entry, E^{n+1} on return.
+        jacobian: another Pic built from the same particles (the fp32 mover) -> pic_jfnk_step_dc
+        (defect correction: residual from this handle, Jacobian-vector products from that one)."""
         assert isinstance(E, np.ndarray) and E.dtype == np.float64
         opts = PicJfnkOpts(rtol, atol, fd_eps, gmres_rtol, max_newton, gmres_restart, max_gmres, 0)
         info = PicJfnkInfo()
-        rc = self._L.pic_jfnk_step(self._h, _ptr(E), C.c_double(dt), C.c_double(tol),
-                                   C.byref(opts), C.byref(info))
+        if jacobian is None:
+            rc = self._L.pic_jfnk_step(self._h, _ptr(E), C.c_double(dt), C.c_double(tol),
+                                       C.byref(opts), C.byref(info))
+        else:
+            rc = self._L.pic_jfnk_step_dc(self._h, jacobian._h, _ptr(E), C.c_double(dt),
+                                          C.c_double(tol), C.byref(opts), C.byref(info))
         d = info.as_dict()
         d["rc"] = rc
         if rc != 0 and not (rc == -5 and not d["converged"]):

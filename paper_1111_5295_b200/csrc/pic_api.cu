@@ -174,6 +174,14 @@ thread_local std::string g_init_err;
 
 using namespace picb200;
 
+namespace {
+template <typename TS, typename TD>
+void convert_arr(pic_handle* d, long long n, const void* a, void* b) {
+  picb200::convert_kernel<TS, TD><<<grid_for(n), 256, 0, d->stream>>>(n, (const TS*)a, (TD*)b);
+  d->launches++;
+}
+}  // namespace
+
 extern "C" {
 
 int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species, int n_species,
@@ -349,6 +357,40 @@ int pic_residual(pic_handle* h, const double* E_np1, double* resid_out) {
   h->launches++;
   PIC_CUDA(h, cudaGetLastError());
   return from_device(h, h->d_resid, resid_out);
+}
+
+int pic_copy_state(pic_handle* dst, pic_handle* src) {
+  if (!dst || !src) return PIC_ERR_ARG;
+  if (dst == src) return PIC_OK;
+  if (dst->grid.n_cells != src->grid.n_cells || dst->grid.length != src->grid.length ||
+      dst->sp.size() != src->sp.size())
+    return set_err(dst, PIC_ERR_ARG, "pic_copy_state: grids or species differ");
+  for (size_t s = 0; s < src->sp.size(); ++s)
+    if (dst->sp[s].n != src->sp[s].n) return set_err(dst, PIC_ERR_ARG, "pic_copy_state: particle counts differ");
+  // src's pending work must be complete before dst's stream reads its buffers
+  PIC_CUDA(dst, cudaStreamSynchronize(src->stream));
+  for (size_t s = 0; s < src->sp.size(); ++s) {
+    const SpeciesState& A = src->sp[s];
+    SpeciesState& Bs = dst->sp[s];
+    if (A.n == 0) continue;
+    const int a = src->cur, b = dst->cur;
+    if (src->elem == 8 && dst->elem == 4) {
+      convert_arr<double, float>(dst, A.n, A.xi[a], Bs.xi[b]);
+      convert_arr<double, float>(dst, A.n, A.v[a], Bs.v[b]);
+    } else if (src->elem == 4 && dst->elem == 8) {
+      convert_arr<float, double>(dst, A.n, A.xi[a], Bs.xi[b]);
+      convert_arr<float, double>(dst, A.n, A.v[a], Bs.v[b]);
+    } else {
+      PIC_CUDA(dst, cudaMemcpyAsync(Bs.xi[b], A.xi[a], src->elem * A.n, cudaMemcpyDeviceToDevice, dst->stream));
+      PIC_CUDA(dst, cudaMemcpyAsync(Bs.v[b], A.v[a], src->elem * A.n, cudaMemcpyDeviceToDevice, dst->stream));
+    }
+    PIC_CUDA(dst, cudaMemcpyAsync(Bs.cell[b], A.cell[a], sizeof(int32_t) * A.n, cudaMemcpyDeviceToDevice, dst->stream));
+    PIC_CUDA(dst, cudaMemcpyAsync(Bs.id[b], A.id[a], sizeof(uint32_t) * A.n, cudaMemcpyDeviceToDevice, dst->stream));
+    Bs.nx = A.nx; Bs.nv = A.nv; Bs.vmean = A.vmean; Bs.vinv = A.vinv;
+  }
+  PIC_CUDA(dst, cudaGetLastError());
+  dst->have_np1 = false;
+  return PIC_OK;
 }
 
 int pic_commit(pic_handle* h) {

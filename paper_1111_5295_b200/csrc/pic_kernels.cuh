@@ -246,6 +246,14 @@ static __global__ void unpermute_counts_kernel(long long n, const uint32_t* __re
   }
 }
 
+// pic_copy_state: element-wise conversion between the precisions of two handles.
+template <typename TS, typename TD>
+__global__ void convert_kernel(long long n, const TS* __restrict__ a, TD* __restrict__ b) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x)
+    b[i] = (TD)a[i];
+}
+
 // sum_p v_p^2 (fp64), one atomic per block.
 template <typename T>
 __global__ void sumsq_kernel(long long n, const T* __restrict__ v, double* __restrict__ out) {

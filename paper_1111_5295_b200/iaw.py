@@ -25,7 +25,7 @@ def gauss_field(rho, dx):
 
 
 def run(config=1, steps=10, precision=None, rtol=None, ppc=None, flags=B.PIC_FLAG_VSORT,
-        verbose=True):
+        verbose=True, defect_correction=False):
     cfg = (W.config1(ppc or 2000) if config == 1 else W.config4(ppc or 4000))
     precision = precision or ("fp64" if config == 1 else "fp32")
     # A-14: 1e-8 needs the fp64 mover; the fp32 mover stalls below ~2e-4
@@ -33,6 +33,9 @@ def run(config=1, steps=10, precision=None, rtol=None, ppc=None, flags=B.PIC_FLA
     ng, L, dt = cfg["n_cells"], cfg["length"], cfg["dt"]
     dx = L / ng
     pic = B.Pic(ng, L, cfg["species"], precision=precision, cn_mode="direct", flags=flags)
+    # defect correction: residual from `pic` (fp64), J w from an fp32 twin
+    jac = (B.Pic(ng, L, cfg["species"], precision="fp32", cn_mode="direct", flags=flags)
+           if defect_correction else None)
     E = gauss_field(pic.rho(B.PIC_STATE_N), dx)
     w_m = [sp["w_q"] / sp["q_over_m"] for sp in cfg["species"]]
 
@@ -52,14 +55,15 @@ def run(config=1, steps=10, precision=None, rtol=None, ppc=None, flags=B.PIC_FLA
     hist = []
     for n in range(steps):
         t0 = time.perf_counter()
-        info = pic.jfnk_step(E, dt, rtol=rtol)
+        info = pic.jfnk_step(E, dt, rtol=rtol, jacobian=jac)
         wall = time.perf_counter() - t0
         if not info["converged"]:
             raise RuntimeError(f"step {n}: Newton did not converge: {info}")
         d = diagnostics()
         etot = sum(d["ke"]) + d["field"]
         rec = dict(step=n + 1, newton=info["newton_its"], gmres=info["gmres_its"],
-                   mover_calls=info["mover_calls"], resid0=info["resid0"], resid=info["resid"],
+                   mover_calls=info["mover_calls"], mover_calls_resid=info["mover_calls_resid"],
+                   resid0=info["resid0"], resid=info["resid"],
                    dE_rel=(etot - e0) / e0, gauss=d["gauss"], momentum=d["momentum"],
                    ke=d["ke"], field=d["field"], wall_s=wall)
         hist.append(rec)
@@ -69,7 +73,9 @@ def run(config=1, steps=10, precision=None, rtol=None, ppc=None, flags=B.PIC_FLA
                   f"gauss {rec['gauss']:.2e} P {rec['momentum']:+.3e} wall {wall * 1e3:.1f} ms",
                   flush=True)
     pic.close()
-    return dict(config=config, precision=precision, rtol=rtol, n_cells=ng,
+    if jac is not None:
+        jac.close()
+    return dict(config=config, precision=precision + ("+fp32 J" if defect_correction else ""), rtol=rtol, n_cells=ng,
                 particles=[int(sp["x"].shape[0]) for sp in cfg["species"]], dt=dt, e0=e0,
                 history=hist)
 
@@ -81,14 +87,17 @@ def main():
     ap.add_argument("--precision", default=None, choices=["fp32", "fp64"])
     ap.add_argument("--rtol", type=float, default=None)
     ap.add_argument("--ppc", type=int, default=None, help="particles per cell per species")
+    ap.add_argument("--defect-correction", action="store_true",
+                    help="fp64 residual, fp32 Jacobian-vector products (needs --precision fp64)")
     ap.add_argument("--json", default=None, help="write the history to this file")
     a = ap.parse_args()
-    out = run(a.config, a.steps, a.precision, a.rtol, a.ppc)
+    out = run(a.config, a.steps, a.precision, a.rtol, a.ppc, defect_correction=a.defect_correction)
     h = out["history"]
     print(json.dumps(dict(config=out["config"], precision=out["precision"], rtol=out["rtol"],
                           steps=len(h), newton_mean=float(np.mean([r["newton"] for r in h])),
                           gmres_mean=float(np.mean([r["gmres"] for r in h])),
                           mover_calls_mean=float(np.mean([r["mover_calls"] for r in h])),
+                          mover_calls_resid_mean=float(np.mean([r["mover_calls_resid"] for r in h])),
                           max_abs_dE_rel=float(np.max(np.abs([r["dE_rel"] for r in h]))),
                           max_gauss=float(np.max([r["gauss"] for r in h])),
                           wall_ms_per_step=float(1e3 * np.mean([r["wall_s"] for r in h])))))

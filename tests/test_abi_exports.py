@@ -30,7 +30,7 @@ def test_struct_sizes():
     assert C.sizeof(B.PicParams) == 48
     assert C.sizeof(B.PicStats) == 80
     assert C.sizeof(B.PicJfnkOpts) == 48
-    assert C.sizeof(B.PicJfnkInfo) == 32
+    assert C.sizeof(B.PicJfnkInfo) == 40
 
 
 def test_no_cpu_fallback():

@@ -108,3 +108,38 @@ def test_jfnk_steps_iaw(oracle):
     # energy conserved to the nonlinear tolerance level
     assert abs(energy() - e0) / e0 < 1e-8
     pic.close()
+
+
+def test_defect_correction_matches_fp64(oracle):
+    """S8(f) #2 / P:325-331: residual from the fp64 mover, Jacobian-vector products from the fp32
+    mover: the converged fields must equal the all-fp64 solve to the nonlinear tolerance, with
+    most mover calls in fp32."""
+    from paper_1111_5295_b200 import binding as B
+    from paper_1111_5295_b200.iaw import gauss_field
+    cfg = W._iaw("iaw-dc", 64, 500, 1.0, W.DEFAULT_SEED)
+    ng, L, dt = cfg["n_cells"], cfg["length"], cfg["dt"]
+    dx = L / ng
+    ref = B.Pic(ng, L, cfg["species"], precision="fp64", flags=B.PIC_FLAG_VSORT)
+    h64 = B.Pic(ng, L, cfg["species"], precision="fp64", flags=B.PIC_FLAG_VSORT)
+    h32 = B.Pic(ng, L, cfg["species"], precision="fp32", flags=B.PIC_FLAG_VSORT)
+    E_ref = gauss_field(ref.rho(B.PIC_STATE_N), dx)
+    E_dc = E_ref.copy()
+    e0 = float(h64.kinetic_energy(B.PIC_STATE_N).sum() + 0.5 * dx * np.sum(E_dc * E_dc))
+    for step in range(3):
+        ia = ref.jfnk_step(E_ref, dt, rtol=1e-9)
+        ib = h64.jfnk_step(E_dc, dt, rtol=1e-9, jacobian=h32)
+        assert ia["converged"] == 1 and ib["converged"] == 1, (ia, ib)
+        err = np.linalg.norm(E_dc - E_ref) / np.linalg.norm(E_ref)
+        print(f"[dc] step {step}: fp64 newton={ia['newton_its']} calls={ia['mover_calls']} | "
+              f"dc newton={ib['newton_its']} calls={ib['mover_calls']} of which fp64 "
+              f"{ib['mover_calls_resid']} |R|={ib['resid']:.2e} |E_dc-E_64|/|E|={err:.2e}")
+        assert err < 1e-7
+        assert ib["mover_calls_resid"] <= 0.5 * ib["mover_calls"]      # most calls are fp32
+        # the fp32 handle follows the committed fp64 state (converted), in the same order
+        a, b = h64.get_particles(0, B.PIC_STATE_N), h32.get_particles(0, B.PIC_STATE_N)
+        assert np.array_equal(a["cell"], b["cell"])
+        assert np.max(np.abs(a["v"] - b["v"])) <= 1e-6 * np.max(np.abs(a["v"]))
+    e1 = float(h64.kinetic_energy(B.PIC_STATE_N).sum() + 0.5 * dx * np.sum(E_dc * E_dc))
+    assert abs(e1 - e0) / e0 < 1e-8
+    for p in (ref, h64, h32):
+        p.close()
