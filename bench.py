@@ -150,6 +150,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1 << 19)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: phase-space cell)")
+    ap.add_argument("--vp", action="store_true",
+                    help="Vlasov-Poisson variant of the mover: orbits without the current deposit (P:281)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -179,6 +181,8 @@ def main():
     n_p = sp["x"].shape[0]
     stream = torch.cuda.current_stream().cuda_stream
     flags = 0 if args.no_vsort else B.PIC_FLAG_VSORT
+    if args.vp:
+        flags |= B.PIC_FLAG_NO_DEPOSIT
     pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=args.precision,
                 cn_mode=args.cn_mode, flags=flags, stream=stream)
     ng = cfg["n_cells"]
@@ -270,6 +274,7 @@ def main():
         "dtype": "f32" if args.precision == "fp32" else "f64", "data": "synthetic",
         "config": {"workload": f"{args.workload}: {ng} cells, {n_p} particles/GPU, dt={dt}",
                    "precision": args.precision, "cn_mode": args.cn_mode,
+                   "variant": "VP (no current deposit, P:281)" if args.vp else "VA (orbit-averaged current)",
                    "binning": "cell" if args.no_vsort else "phase-space cell: cell + offset class + velocity class (P:242-250)",
                    "substeps_per_particle": n_sub / max(n_p, 1),
                    "crossing_fraction": n_cross / max(n_sub, 1),

@@ -49,6 +49,9 @@ enum {
   PIC_FLAG_DIAG = 2,       /* count anomalies (kappa cap, clamped roots, ...) in pic_stats     */
   PIC_FLAG_NO_STORE = 4,   /* Krylov calls: skip the state-(n+1) store, only jbar is wanted    */
   PIC_FLAG_VSORT = 8,      /* bin by (cell, |v| class) instead of cell only        */
+  PIC_FLAG_NO_DEPOSIT = 32,/* Vlasov-Poisson variant of the mover: no
+                              current deposit during the orbit (jbar comes back as 0); the
+                              charge density of state n+1 is then pic_rho(PIC_STATE_NP1)      */
   PIC_FLAG_DEPOSIT_PER_VISIT = 16 /* deposit per cell visit with shared fp64 atomics
                               instead of the default end-point form (D:5); same jbar to rounding */
 };

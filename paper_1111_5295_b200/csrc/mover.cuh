@@ -58,6 +58,7 @@ struct MoverArgs {
   int32_t tile;                // particles per claimed index range (multiple of 32)
   int32_t refill_threshold;    // parked lanes needed before a refill
   int32_t wrap_mask;           // n_cells - 1 if n_cells is a power of two, else 0
+  int32_t deposit;             // 0 = VP variant: orbits only, no current deposit
   double qm_over_dx;           // (q/m)/dx
   T dx, inv_dx;
   T c_abs;                     // sqrt(2 eps_a / dx):   dtau_abs = c_abs / sqrt(|A| + |dA u|)
@@ -450,7 +451,8 @@ mover_kernel(const MoverArgs<T> a) {
             const int32_t c1 = POW2 ? (p.c & a.wrap_mask) : p.c;
             const int32_t k = POW2 ? (p.c - p.c0) : (int32_t)(2u * p.nr - p.nc);
             if (PER_VISIT) deposit_visit<T>(sF, a.n_cells, c1, p.xa, p.xi);
-            else deposit_endpoint(sF, sD, a.n_cells, acc, et, p.c0, (double)p.xa, c1, (double)p.xi, k);
+            else if (a.deposit)
+              deposit_endpoint(sF, sD, a.n_cells, acc, et, p.c0, (double)p.xa, c1, (double)p.xi, k);
             p.c = c1;
             if (a.xi1) {
               a.xi1[p.idx] = p.xi;

@@ -72,6 +72,7 @@ void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const do
   a.max_substeps = P.max_substeps;
   a.picard_max = P.picard_max;
   a.tile = S.tile;
+  a.deposit = (P.flags & PIC_FLAG_NO_DEPOSIT) ? 0 : 1;
   a.wrap_mask = (h->grid.n_cells > 1 && (h->grid.n_cells & (h->grid.n_cells - 1)) == 0)
                     ? h->grid.n_cells - 1 : 0;
   // velocity-sorted warps finish in bunches: wait for a larger bunch before the refill block
@@ -93,7 +94,7 @@ void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const do
   const bool direct = P.cn_mode == PIC_CN_DIRECT;
   // the counting build: exact per-particle sub-step counts and anomaly counters
   const bool diag = (P.flags & (PIC_FLAG_DIAG | PIC_FLAG_COUNTS)) != 0;
-  const bool per_visit = (P.flags & PIC_FLAG_DEPOSIT_PER_VISIT) != 0;
+  const bool per_visit = (P.flags & PIC_FLAG_DEPOSIT_PER_VISIT) != 0 && !(P.flags & PIC_FLAG_NO_DEPOSIT);
   dim3 g(S.grid_blocks), b(kBlock);
   with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, [&](auto k) {
     k<<<g, b, h->smem_bytes, h->stream>>>(a);

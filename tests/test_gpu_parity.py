@@ -147,6 +147,34 @@ def test_non_power_of_two_grid(G, oracle, precision, n_cells):
         m["gpu"]["pic"].close()
 
 
+# ---- Vlasov-Poisson variant: orbits without the current deposit, rho at the end
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_vp_variant_no_deposit(G, oracle, precision):
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config2(n=60_013)
+    sp = cfg["species"][0]
+    dx = cfg["length"] / cfg["n_cells"]
+    va = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=precision, flags=B.PIC_FLAG_VSORT)
+    vp = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=precision,
+               flags=B.PIC_FLAG_VSORT | B.PIC_FLAG_NO_DEPOSIT)
+    ja = va.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+    jp = vp.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+    assert np.all(jp == 0.0) and np.any(ja != 0.0)
+    a, b = va.get_particles(0, B.PIC_STATE_NP1), vp.get_particles(0, B.PIC_STATE_NP1)
+    for k in ("x", "v", "cell", "xi"):
+        assert np.array_equal(a[k], b[k]), k                      # same orbits
+    # charge density of state n+1 (quadratic spline, A-10) against the oracle's O11 on the
+    # kernel's own end state, and continuity ties it to the VA run's jbar
+    rho1 = vp.rho(B.PIC_STATE_NP1)
+    ref = oracle.rho(cfg["n_cells"], cfg["length"], sp["w_q"], b["cell"], b["xi"] * dx)
+    assert G.rel_l2(rho1, ref) < 1e-12
+    rho0 = vp.rho(B.PIC_STATE_N)
+    div = cfg["dt"] * (np.roll(ja, -1) - ja) / dx
+    assert np.linalg.norm(rho1 - rho0 + div) <= 1e-10 * np.linalg.norm(div)
+    va.close()
+    vp.close()
+
+
 # ---- long orbits: many wraps of the periodic ring (end-point deposit: whole turns) -----------
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_ring_wraps(G, oracle, precision):
