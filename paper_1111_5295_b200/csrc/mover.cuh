@@ -98,6 +98,13 @@ template <> struct Prim<double> {
   static __device__ __forceinline__ double div(double a, double b) { return a / b; }
 };
 
+// xi in [0,1] (inclusive, A-5).  fp32: one unsigned compare of the bit pattern (non-negative
+// floats order like their bits; a set sign bit or a NaN compares above 1.0f's pattern).
+template <typename T> __device__ __forceinline__ bool in_unit(T x);
+template <> __device__ __forceinline__ bool in_unit<float>(float x) {
+  return __float_as_uint(x) <= 0x3f800000u; }
+template <> __device__ __forceinline__ bool in_unit<double>(double x) { return x >= 0.0 && x <= 1.0; }
+
 template <typename T> __device__ __forceinline__ T tabs(T x);
 template <> __device__ __forceinline__ float tabs<float>(float x) { return fabsf(x); }
 template <> __device__ __forceinline__ double tabs<double>(double x) { return fabs(x); }
@@ -289,15 +296,16 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
   const T A = fma(p.dA, p.xi, p.AL);
   const T absA = tabs(A);
   const T d = Prim<T>::rsqrt(absA + tabs(p.dA * p.u));
-  T dtau = tmax(a.c_abs * d, (a.c_rel * (absA + tabs(p.u))) * (d * d));
+  T dtau = tmax(a.c_abs, (a.c_rel * (absA + tabs(p.u))) * d) * d;
   if (DIAG && dtau > p.cap) diag[ST_KAPPA_CAP]++;
   dtau = tmin(tmin(dtau, p.cap), p.r);
 
   // ---- a3 / O5: Crank-Nicolson step over dtau with the linear field of the current cell (A-4).
+  const T h = T(0.5) * dtau;
   T u1;
   if (CN_DIRECT) {
     // Eq. 11: kappa = a' dtau^2/4;  u' = [A dtau + (1+kappa) u] / (1-kappa).
-    const T kappa = (T(0.25) * p.dA) * (dtau * dtau);
+    const T kappa = p.dA * (h * h);
     const T num = fma(A, dtau, fma(kappa, p.u, p.u));
     u1 = Prim<T>::div(num, T(1) - kappa);
   } else {
@@ -306,7 +314,7 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     T uk = p.u;
     int it = 0;
     for (;;) {
-      const T xim = fma(T(0.25) * dtau, p.u + uk, p.xi);
+      const T xim = fma(T(0.5) * h, p.u + uk, p.xi);
       const T Am = fma(p.dA, xim, p.AL);
       const T un = fma(dtau, Am, p.u);
       ++it;
@@ -318,12 +326,12 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     picard_its += it;
     u1 = uk;
   }
-  const T xi1 = fma(T(0.5) * dtau, p.u + u1, p.xi);   // Eq. 9
+  const T xi1 = fma(h, p.u + u1, p.xi);               // Eq. 9
   // exact per-particle sub-step count only in the counting build (DIAG); a parked lane (r = 0)
   // takes a zero-length step that changes nothing and is not counted
   if (DIAG) { if (p.r > T(0)) p.ns++; }
 
-  if (xi1 >= T(0) && xi1 <= T(1)) {
+  if (in_unit<T>(xi1)) {
     // ---- O6: accept (inclusive, A-5).
     p.xi = xi1;
     p.u = u1;
