@@ -52,6 +52,9 @@ enum {
   PIC_FLAG_NO_DEPOSIT = 32,/* Vlasov-Poisson variant of the mover: no
                               current deposit during the orbit (jbar comes back as 0); the
                               charge density of state n+1 is then pic_rho(PIC_STATE_NP1)      */
+  PIC_FLAG_ONE_PER_LANE = 64, /* fp32 only: run the one-particle-per-lane kernel also where the
+                              default two-particles-per-lane packed-FP32 kernel (FFMA2) applies;
+                              both give bit-identical orbits (A/B timing, tests)               */
   PIC_FLAG_DEPOSIT_PER_VISIT = 16 /* deposit per cell visit with shared fp64 atomics
                               instead of the default end-point form (D:5); same jbar to rounding */
 };
@@ -146,7 +149,8 @@ int pic_get_counts(pic_handle* h, int species, uint32_t* n_sub, uint32_t* n_cros
 /* pic_get_stats — totals of the last move (synchronises the stream). */
 int pic_get_stats(pic_handle* h, pic_stats* out);
 
-/* pic_set_flags — replace pic_params.flags (COUNTS / DIAG / NO_STORE) between calls. */
+/* pic_set_flags — replace pic_params.flags (COUNTS / DIAG / NO_STORE / NO_DEPOSIT /
+ * ONE_PER_LANE / DEPOSIT_PER_VISIT) between calls. */
 int pic_set_flags(pic_handle* h, uint32_t flags);
 
 /* pic_kinetic_energy — sum_p w_m v_p^2 / 2 per species (w_m = w_q / (q/m)) of state `which`,

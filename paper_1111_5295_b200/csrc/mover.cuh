@@ -279,6 +279,36 @@ __device__ __forceinline__ void warp_deposit_end(double* __restrict__ sF, int32_
   }
 }
 
+// ---- a8: one flush per block.  Inclusive prefix sum of the difference array over the
+// faces (each thread owns a contiguous chunk), then scaled block sums -> this block's row of
+// `partial`.  Called by every thread of the block after its warps have left the particle loop.
+template <typename T>
+__device__ __forceinline__ void block_flush(const MoverArgs<T>& a, const double* __restrict__ sF,
+                                            const int32_t* __restrict__ sD, int32_t* s_wtot) {
+  const int lane = threadIdx.x & 31;
+  __syncthreads();
+  const int per = (a.n_cells + (int)blockDim.x - 1) / (int)blockDim.x;
+  const int fb = min((int)threadIdx.x * per, a.n_cells), fe = min(fb + per, a.n_cells);
+  int32_t s = 0;
+  for (int f = fb; f < fe; ++f) s += sD[f];
+  int32_t inc = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int32_t t = __shfl_up_sync(kFull, inc, o);
+    if (lane >= o) inc += t;
+  }
+  const int wid = threadIdx.x >> 5;
+  if (lane == 31) s_wtot[wid] = inc;
+  __syncthreads();
+  int32_t run = inc - s;                       // exclusive within the warp
+  for (int w = 0; w < wid; ++w) run += s_wtot[w];
+  double* row = a.partial + (size_t)blockIdx.x * a.n_cells;
+  for (int f = fb; f < fe; ++f) {
+    run += sD[f];
+    row[f] = a.scale * (sF[f] + (double)run);
+  }
+}
+
 // One sub-step (O3-O8) of the lane's particle: estimate dtau, tentative Crank-Nicolson step in
 // the current cell, accept it if it stays in the cell, otherwise truncate it at the face.
 // CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.  The max_substeps cap (A-9) is checked by the
@@ -533,30 +563,7 @@ mover_kernel(const MoverArgs<T> a) {
     if (lane == 0 && v) atomicAdd(&a.stats[i], (unsigned long long)v);
   }
 
-  // ---- a8: one flush per block.  Inclusive prefix sum of the difference array over
-  // the faces (each thread owns a contiguous chunk), then scaled block sums -> this block's
-  // row of `partial`.
-  __syncthreads();
-  const int per = (a.n_cells + (int)blockDim.x - 1) / (int)blockDim.x;
-  const int fb = min((int)threadIdx.x * per, a.n_cells), fe = min(fb + per, a.n_cells);
-  int32_t s = 0;
-  for (int f = fb; f < fe; ++f) s += sD[f];
-  int32_t inc = s;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int32_t t = __shfl_up_sync(kFull, inc, o);
-    if (lane >= o) inc += t;
-  }
-  const int wid = threadIdx.x >> 5;
-  if (lane == 31) s_wtot[wid] = inc;
-  __syncthreads();
-  int32_t run = inc - s;                       // exclusive within the warp
-  for (int w = 0; w < wid; ++w) run += s_wtot[w];
-  double* row = a.partial + (size_t)blockIdx.x * a.n_cells;
-  for (int f = fb; f < fe; ++f) {
-    run += sD[f];
-    row[f] = a.scale * (sF[f] + (double)run);
-  }
+  block_flush<T>(a, sF, sD, s_wtot);
 }
 
 }  // namespace picb200

@@ -313,7 +313,7 @@ int pic_move_accumulate(pic_handle* h, const double* E_n, const double* E_np1, d
   int row = 0;
   for (int s = 0; s < ns; ++s) {
     if ((rc = launch_mover(h, s, dEn, dEp, dt, tol, row)) != PIC_OK) return rc;
-    row += h->sp[s].grid_blocks;
+    row += h->sp[s].last_blocks;
   }
   PIC_CUDA(h, cudaEventRecord(h->ev1, h->stream));
   const int32_t ng = h->grid.n_cells;

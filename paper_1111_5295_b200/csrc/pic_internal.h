@@ -23,7 +23,10 @@ struct SpeciesState {
   int32_t nx = 1, nv = 1;                 // offset / velocity classes of the sort key (1 = cell only)
   double vmean = 0, vinv = 0;
   int grid_blocks = 0;                    // mover launch shape for this species
+  int grid_blocks2 = 0;                   // same for the two-per-lane fp32 kernel (0 = not usable)
+  int last_blocks = 0;                    // blocks (= rows of `partial`) of the last launch
   int tile = 0;
+  int tile2 = 0;
 };
 
 }  // namespace picb200
@@ -41,6 +44,7 @@ struct pic_handle {
   int sm_count = 0;
   int blocks_per_sm = 2;
   size_t smem_bytes = 0;
+  size_t smem_bytes2 = 0;      // two-per-lane fp32 kernel (mover2.cuh)
   // device scratch
   double* dE_n = nullptr;      // [n_cells] staging for host E^n / stored E^n of pic_set_step
   double* dE_step = nullptr;   // [n_cells] E^n of pic_set_step

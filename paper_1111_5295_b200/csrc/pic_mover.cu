@@ -4,6 +4,7 @@
 #include <cmath>
 
 #include "mover.cuh"
+#include "mover2.cuh"
 #include "pic_internal.h"
 
 namespace picb200 {
@@ -50,7 +51,7 @@ int occupancy(size_t bytes) {
 }
 
 template <typename T>
-void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const double* dE_np1,
+void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* dE_np1,
               double dt, double tol, int row0, int s) {
   const pic_params& P = h->params;
   const double dx = h->grid.length / h->grid.n_cells;
@@ -95,6 +96,18 @@ void launch_t(pic_handle* h, const SpeciesState& S, const double* dE_n, const do
   // the counting build: exact per-particle sub-step counts and anomaly counters
   const bool diag = (P.flags & (PIC_FLAG_DIAG | PIC_FLAG_COUNTS)) != 0;
   const bool per_visit = (P.flags & PIC_FLAG_DEPOSIT_PER_VISIT) != 0 && !(P.flags & PIC_FLAG_NO_DEPOSIT);
+  if constexpr (sizeof(T) == 4) {
+    // production fp32 path: two particles per lane, packed FP32 (mover2.cuh)
+    if (direct && !diag && !per_visit && a.wrap_mask != 0 && S.grid_blocks2 > 0 &&
+        !(P.flags & PIC_FLAG_ONE_PER_LANE)) {
+      a.refill_threshold = (S.nv > 1 || S.nx > 1) ? kRefill2Vsort : kRefill2;
+      a.tile = S.tile2;
+      S.last_blocks = S.grid_blocks2;
+      mover2_kernel<<<dim3(S.grid_blocks2), dim3(kBlock2), h->smem_bytes2, h->stream>>>(a);
+      return;
+    }
+  }
+  S.last_blocks = S.grid_blocks;
   dim3 g(S.grid_blocks), b(kBlock);
   with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, [&](auto k) {
     k<<<g, b, h->smem_bytes, h->stream>>>(a);
@@ -133,13 +146,36 @@ int mover_configure(pic_handle* h) {
     S.tile = (int)tile;
     rows += S.grid_blocks;
   }
+  // two-per-lane fp32 kernel: power-of-two grids whose 28 B per cell leave two blocks per SM
+  const int32_t ng = h->grid.n_cells;
+  if (h->elem == 4 && ng > 1 && (ng & (ng - 1)) == 0) {
+    const size_t b2 = mover2_smem_bytes(ng);
+    int occ2 = 0;
+    if (b2 <= 113 * 1024 &&
+        cudaFuncSetAttribute(mover2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b2) == cudaSuccess &&
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, mover2_kernel, kBlock2, b2) == cudaSuccess &&
+        occ2 >= 2) {
+      h->smem_bytes2 = b2;
+      for (auto& S : h->sp) {
+        const long long full = (long long)h->sm_count * occ2;
+        const long long want = (S.n + kBlock2 * 8 - 1) / (kBlock2 * 8);
+        S.grid_blocks2 = (int)std::max<long long>(1, std::min<long long>(std::min(full, want), S.grid_blocks));
+        const long long warps = (long long)S.grid_blocks2 * (kBlock2 / 32);
+        long long tile = S.n / (warps * 8);
+        tile = std::max<long long>(64, std::min<long long>(PIC_TILE_MAX, tile / 64 * 64));
+        S.tile2 = (int)tile;
+      }
+    } else {
+      cudaGetLastError();
+    }
+  }
   h->total_rows = rows;
   return PIC_OK;
 }
 
 int launch_mover(pic_handle* h, int s, const double* dE_n, const double* dE_np1, double dt,
                  double tol, int row0) {
-  const SpeciesState& S = h->sp[s];
+  SpeciesState& S = h->sp[s];
   if (h->elem == 4) launch_t<float>(h, S, dE_n, dE_np1, dt, tol, row0, s);
   else launch_t<double>(h, S, dE_n, dE_np1, dt, tol, row0, s);
   h->launches++;

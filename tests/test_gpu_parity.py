@@ -123,6 +123,31 @@ def test_fast_build_matches_counting_build(G, precision):
     assert sc["n_sub"] <= sf["n_sub"] < sc["n_sub"] + 4 * 120_007   # grouped upper bound
 
 
+# ---- the production fp32 kernel (two particles per lane, packed FFMA2/FMUL2/FADD2, mover2.cuh)
+# against the one-particle-per-lane kernel: same arithmetic in the same order => identical orbits
+@pytest.mark.parametrize("case", ["cfg0", "cfg2-vsort", "cfg2-cell", "cfg3-vsort", "cfg2-odd-tail"])
+def test_two_per_lane_matches_one_per_lane(G, case):
+    from paper_1111_5295_b200 import binding as B
+    cfg = {"cfg0": lambda: W.config0(), "cfg2-vsort": lambda: W.config2(n=150_001),
+           "cfg2-cell": lambda: W.config2(n=90_001), "cfg3-vsort": lambda: W.config3(n=20_011),
+           "cfg2-odd-tail": lambda: W.config2(n=65)}[case]()
+    base = 0 if case in ("cfg0", "cfg2-cell") else B.PIC_FLAG_VSORT
+    sp = cfg["species"][0]
+    out = {}
+    for name, flags in (("two", base), ("one", base | B.PIC_FLAG_ONE_PER_LANE)):
+        pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp32", flags=flags)
+        j = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+        j2 = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])      # repeatable
+        assert G.rel_l2(j2, j) < 1e-13
+        out[name] = (pic.get_particles(0, B.PIC_STATE_NP1), j, pic.get_stats())
+        pic.close()
+    (p2, j2, s2), (p1, j1, s1) = out["two"], out["one"]
+    for k in ("x", "v", "cell", "xi"):
+        assert np.array_equal(p2[k], p1[k]), k            # bit-identical orbits
+    assert np.any(j1 != 0.0) and G.rel_l2(j2, j1) < 1e-13  # same deposits, atomics in any order
+    assert s2["n_sub"] == s1["n_sub"]                      # same grouped sub-step count
+
+
 # ---- grids whose cell count is not a power of two take the generic wrap path --------------------
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 @pytest.mark.parametrize("n_cells", [3, 48, 100])
