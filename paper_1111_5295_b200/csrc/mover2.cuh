@@ -257,8 +257,15 @@ mover2_kernel(const MoverArgs<float> a) {
                        tot_sub, capped);
         refill_slot<1>(a, sF, sD, sC, p, acc, et1, (uint32_t)(n0 + __popc(pk1 & lt_mask)), next, end,
                        tot_sub, capped);
+        // the two slots of a lane mostly end in the same cell: add them up first, then one
+        // warp-level pass (a second one only if some lane's slots ended in different cells)
+        if (et0.pending && et1.pending && et0.cell == et1.cell) {
+          et0.e0 += et1.e0; et0.e1 += et1.e1; et1.pending = false;
+        } else if (!et0.pending && et1.pending) {
+          et0 = et1; et1.pending = false;
+        }
         warp_deposit_end(sF, a.n_cells, lane, et0);
-        warp_deposit_end(sF, a.n_cells, lane, et1);
+        if (__any_sync(kFull, et1.pending)) warp_deposit_end(sF, a.n_cells, lane, et1);
         next = ((uint32_t)n_parked < end - next) ? next + (uint32_t)n_parked : end;
         if (exhausted && n_parked == 64) break;
       }
