@@ -35,7 +35,7 @@ UNIT = "sub-steps/s"
 OPS_INCELL, OPS_CROSS = 43.0, 72.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one mover launch from the committed
 # `ncu --set full` capture (profiles/r1_mover_ncu.md); known only for the default workload.
-NCU_TRAFFIC_BYTES = {("cfg2", 100_000_000, "fp32"): 2.369e9}
+NCU_TRAFFIC_BYTES = {("cfg2", 100_000_000, "fp32"): 2.366e9}
 
 
 def _workload(name, n, seed):
@@ -150,6 +150,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1 << 19)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: phase-space cell)")
+    ap.add_argument("--one-per-lane", action="store_true",
+                    help="fp32: the one-particle-per-lane kernel instead of the packed two-per-lane one")
     ap.add_argument("--vp", action="store_true",
                     help="Vlasov-Poisson variant of the mover: orbits without the current deposit (P:281)")
     args = ap.parse_args()
@@ -183,6 +185,8 @@ def main():
     flags = 0 if args.no_vsort else B.PIC_FLAG_VSORT
     if args.vp:
         flags |= B.PIC_FLAG_NO_DEPOSIT
+    if args.one_per_lane:
+        flags |= B.PIC_FLAG_ONE_PER_LANE
     pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=args.precision,
                 cn_mode=args.cn_mode, flags=flags, stream=stream)
     ng = cfg["n_cells"]
@@ -266,6 +270,7 @@ def main():
     else:
         peak_gops = sms * 64 * 2 * sm_max_mhz * 1e-3       # FP64: 64 DFMA lanes per SM
     ops_per_launch = OPS_INCELL * (n_sub - n_cross) + OPS_CROSS * n_cross
+    kernel_name = pic.last_kernel()        # the kernel the timed launches ran (library's word)
     achieved = ops_per_launch / (k_ms * 1e-3) * 1e-9
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -290,7 +295,7 @@ def main():
                      "traffic": NCU_TRAFFIC_BYTES.get((args.workload, n_p, args.precision)),
                      "traffic_unit": "bytes per launch (ncu dram read+write); algorithmic %d"
                                      % (n_p * (24 if args.precision == "fp32" else 40)),
-                     "kernel": "mover_kernel", "kernel_ms": k_ms,
+                     "kernel": kernel_name, "kernel_ms": k_ms,
                      "ops_per_launch": ops_per_launch,
                      "peak_source": "derived: SMs x lanes x 2 x sm_max_mhz (DESIGN.md 6)",
                      "hbm_gbs_algorithmic": n_p * (24 if args.precision == "fp32" else 40) / (k_ms * 1e-3) * 1e-9},

@@ -206,6 +206,10 @@ int pic_copy_state(pic_handle* dst, pic_handle* src);
 
 int pic_destroy(pic_handle* h);
 const char* pic_last_error(const pic_handle* h);
+/* Name of the mover kernel the last pic_move_accumulate launched (static string): "mover2_kernel"
+ * (fp32, two particles per lane, packed FP32; csrc/mover2.cuh) or "mover_kernel" (csrc/mover.cuh);
+ * "" before the first move.  For bench lines and profiles. */
+const char* pic_last_kernel(const pic_handle* h);
 /* Library/device identification for logs: fills buf with e.g. "pic_b200 sm_100a ...". */
 int pic_version(char* buf, int buflen);
 

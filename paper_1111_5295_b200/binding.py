@@ -27,7 +27,7 @@ PIC_ERR_SUBSTEP_CAP = -4
 EXPORTS = ["pic_init", "pic_move_accumulate", "pic_set_step", "pic_residual", "pic_commit",
            "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_set_flags",
            "pic_kinetic_energy", "pic_rho", "pic_jfnk_step", "pic_jfnk_step_dc",
-           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_version"]
+           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_last_kernel", "pic_version"]
 
 
 class PicGrid(C.Structure):
@@ -94,6 +94,8 @@ def load():
         L = C.CDLL(path)
         L.pic_last_error.restype = C.c_char_p
         L.pic_last_error.argtypes = [C.c_void_p]
+        L.pic_last_kernel.restype = C.c_char_p
+        L.pic_last_kernel.argtypes = [C.c_void_p]
         for name in EXPORTS:
             getattr(L, name)  # fail loudly on a missing symbol
         _lib = L
@@ -217,6 +219,9 @@ class Pic:
         st = PicStats()
         self._chk(self._L.pic_get_stats(self._h, C.byref(st)))
         return st.as_dict()
+
+    def last_kernel(self):
+        return self._L.pic_last_kernel(self._h).decode()
 
     def set_flags(self, flags):
         self._chk(self._L.pic_set_flags(self._h, C.c_uint32(flags)))

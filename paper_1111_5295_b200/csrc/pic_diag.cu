@@ -199,6 +199,7 @@ int pic_destroy(pic_handle* h) {
 }
 
 const char* pic_last_error(const pic_handle* h) { return h ? h->err.c_str() : "invalid handle"; }
+const char* pic_last_kernel(const pic_handle* h) { return h ? h->last_kernel : ""; }
 
 int pic_version(char* buf, int buflen) {
   if (!buf || buflen < 1) return PIC_ERR_ARG;

@@ -62,6 +62,7 @@ struct pic_handle {
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   pic_stats stats{};
   long long launches = 0;
+  const char* last_kernel = "";   // name of the mover kernel of the last launch
   std::string err;
 };
 

@@ -103,11 +103,13 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
       a.refill_threshold = (S.nv > 1 || S.nx > 1) ? kRefill2Vsort : kRefill2;
       a.tile = S.tile2;
       S.last_blocks = S.grid_blocks2;
+      h->last_kernel = "mover2_kernel";
       mover2_kernel<<<dim3(S.grid_blocks2), dim3(kBlock2), h->smem_bytes2, h->stream>>>(a);
       return;
     }
   }
   S.last_blocks = S.grid_blocks;
+  h->last_kernel = "mover_kernel";
   dim3 g(S.grid_blocks), b(kBlock);
   with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, [&](auto k) {
     k<<<g, b, h->smem_bytes, h->stream>>>(a);

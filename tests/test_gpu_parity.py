@@ -139,6 +139,7 @@ def test_two_per_lane_matches_one_per_lane(G, case):
         j = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
         j2 = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])      # repeatable
         assert G.rel_l2(j2, j) < 1e-13
+        assert pic.last_kernel() == ("mover2_kernel" if name == "two" else "mover_kernel")
         out[name] = (pic.get_particles(0, B.PIC_STATE_NP1), j, pic.get_stats())
         pic.close()
     (p2, j2, s2), (p1, j1, s1) = out["two"], out["one"]
