@@ -92,16 +92,27 @@ int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double*
     if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "velocity moments", e);
     const double mean = hm[0] / (double)S.n;
     const double var = hm[1] / (double)S.n - mean * mean;
-    // classes: about 4 particles per phase-space cell, nx <= 8 offset classes, nv <= 1024
+    // classes: about 4 particles per phase-space cell, nx = 8 (or 4) offset classes, nv <= 1024
     // velocity classes (powers of two), at most n_keys keys in all
     const double ppc = (double)S.n / ng;
 #ifndef PIC_NX
 #define PIC_NX 8
 #endif
+#ifndef PIC_NX2
+#define PIC_NX2 4
+#endif
 #ifndef PIC_PPK
 #define PIC_PPK 4
 #endif
-    int32_t nx = PIC_NX, nv = 1;
+    // offset classes: 8 for the one-particle-per-lane kernels; the two-per-lane fp32 kernel
+    // (64 orbits per warp) does better with 4 and twice as fine velocity classes
+    // (profiles/r1_bench.md)
+    const bool pow2 = ng > 1 && (ng & (ng - 1)) == 0;
+    const bool two_per_lane = h->elem == 4 && pow2 && h->params.cn_mode == PIC_CN_DIRECT &&
+        (size_t)ng * 28 <= 113 * 1024 &&
+        !(h->params.flags & (PIC_FLAG_ONE_PER_LANE | PIC_FLAG_DIAG | PIC_FLAG_COUNTS |
+                             PIC_FLAG_DEPOSIT_PER_VISIT));
+    int32_t nx = two_per_lane ? PIC_NX2 : PIC_NX, nv = 1;
 #ifndef PIC_NVMAX
 #define PIC_NVMAX 1024
 #endif

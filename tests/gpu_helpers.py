@@ -63,13 +63,29 @@ def sub_cfg(cfg, subset):
     return out
 
 
-def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=0):
+def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=0, fast=False):
     """Run both sides; return metrics (SURVEY 8(c) 'Parity metrics').  Particles whose
     (n_sub, n_cross, cell) differ are branch flips (A-12): excluded from x/v, counted, and
-    jbar is then recomputed on both sides on the non-flipped subset."""
+    jbar is then recomputed on both sides on the non-flipped subset.
+
+    fast=True: x, v, jbar and continuity are those of the FAST build (no per-particle counters;
+    fp32 on power-of-two grids: mover2_kernel, two particles per lane).  The per-particle
+    counts that identify flips still come from a counting-build run, whose orbits must be
+    bit-identical to the fast build's (asserted here)."""
     dx = cfg["length"] / cfg["n_cells"]
     flags = B.PIC_FLAG_COUNTS | B.PIC_FLAG_DIAG | extra_flags
     g = gpu_run(cfg, precision, cn_mode, flags=flags)
+    if fast:
+        flags = extra_flags
+        gf = gpu_run(cfg, precision, cn_mode, flags=flags)
+        gf["kernel"] = gf["pic"].last_kernel()
+        for a, b in zip(gf["species"], g["species"]):
+            for k in ("x", "v", "cell", "xi"):
+                assert np.array_equal(a[k], b[k]), f"fast build differs from counting build in {k}"
+            a["n_sub"], a["n_cross"] = b["n_sub"], b["n_cross"]
+        gf["stats"] = dict(gf["stats"], n_substep_cap=g["stats"]["n_substep_cap"])
+        g["pic"].close()
+        g = gf
     oc = sub_cfg(cfg, [slice(None)] * len(cfg["species"]))
     ref = oracle_run(o, oc, oracle_params, state=oracle_state_for(cfg, precision))
     m = dict(flips=0, n=0, x=[], v=[], stats=g["stats"], ostats=ref["stats"].as_dict())

@@ -123,6 +123,22 @@ def test_fast_build_matches_counting_build(G, precision):
     assert sc["n_sub"] <= sf["n_sub"] < sc["n_sub"] + 4 * 120_007   # grouped upper bound
 
 
+# ---- the fast build straight against the oracle: fp32 on power-of-two grids this is
+# mover2_kernel (two particles per lane, packed FP32), fp64 the fast build of mover_kernel
+@pytest.mark.parametrize("case", ["cfg0", "cfg2", "cfg2-vsort", "iaw-2species"])
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_fast_build_parity_with_oracle(G, oracle, precision, case):
+    from paper_1111_5295_b200 import binding as B
+    cfg = {"cfg0": lambda: W.config0(), "cfg2": lambda: W.config2(n=100_003),
+           "cfg2-vsort": lambda: W.config2(n=200_003), "iaw-2species": lambda: W.config1(ppc=40)}[case]()
+    extra = B.PIC_FLAG_VSORT if case in ("cfg2-vsort", "iaw-2species") else 0
+    m = G.parity(oracle, cfg, precision, extra_flags=extra, fast=True)
+    _report(f"fast build {case} {precision} [{m['gpu']['kernel']}]", m)
+    assert m["gpu"]["kernel"] == ("mover2_kernel" if precision == "fp32" else "mover_kernel")
+    G.assert_parity(m, precision)
+    m["gpu"]["pic"].close()
+
+
 # ---- the production fp32 kernel (two particles per lane, packed FFMA2/FMUL2/FADD2, mover2.cuh)
 # against the one-particle-per-lane kernel: same arithmetic in the same order => identical orbits
 @pytest.mark.parametrize("case", ["cfg0", "cfg2-vsort", "cfg2-cell", "cfg3-vsort", "cfg2-odd-tail"])
