@@ -89,6 +89,8 @@ template <> struct Prim<float> {
   static __device__ __forceinline__ float sqrt(float x) {   // MUFU.SQRT
     float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
   static __device__ __forceinline__ float div(float a, float b) { return a * rcp(b); }
+  static __device__ __forceinline__ float rsqrt_est(float x) { return rsqrt(x); }
+  static __device__ __forceinline__ float div_unit(float a, float b) { return a * rcp(b); }
 };
 
 template <> struct Prim<double> {
@@ -96,6 +98,27 @@ template <> struct Prim<double> {
   static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
   static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
   static __device__ __forceinline__ double div(double a, double b) { return a / b; }
+  // Estimator only (Eq. 6-8 fix a step SIZE, not a state): MUFU.RSQ64H seed (2^-23) + one
+  // Newton step -> relative error ~3e-14, 4 FP64 instructions instead of 5 + a slow-path test.
+  // x = 0 or denormal gives NaN here (0 * inf); the caller's min/max then yield min(cap, r),
+  // the same limit as A-1's floor on alpha.
+  static __device__ __forceinline__ double rsqrt_est(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-(x * y), y, 1.0);
+    return fma(0.5 * y, e, y);
+  }
+  // a / b for b in (0, 2) and away from 0 (Eq. 11's denominator 1 - kappa, |kappa| <= kappa_max
+  // < 1 by A-2): MUFU.RCP64H seed + two Newton steps, no special-case path; <= 1.5 ulp.
+  static __device__ __forceinline__ double div_unit(double a, double b) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(b));
+    double e = fma(-b, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-b, y, 1.0);
+    y = fma(y, e, y);
+    return a * y;
+  }
 };
 
 // xi in [0,1] (inclusive, A-5).  fp32: one unsigned compare of the bit pattern (non-negative
@@ -108,13 +131,15 @@ template <> __device__ __forceinline__ bool in_unit<double>(double x) { return x
 template <typename T> __device__ __forceinline__ T tabs(T x);
 template <> __device__ __forceinline__ float tabs<float>(float x) { return fabsf(x); }
 template <> __device__ __forceinline__ double tabs<double>(double x) { return fabs(x); }
-// IEEE min/max: a NaN operand is dropped (fmaxf(NaN, x) = x), which the estimator relies on.
+// min/max that drop a NaN in the FIRST operand (tmax(NaN, x) = x), which the estimator (A-1) and
+// the crossing clamp rely on: fp32 uses the IEEE instructions (FMNMX, symmetric); fp64 a compare
+// and select (DSETP + 2 SEL instead of the six-instruction IEEE fmin/fmax sequence).
 template <typename T> __device__ __forceinline__ T tmin(T a, T b);
 template <typename T> __device__ __forceinline__ T tmax(T a, T b);
 template <> __device__ __forceinline__ float tmin<float>(float a, float b) { return fminf(a, b); }
 template <> __device__ __forceinline__ float tmax<float>(float a, float b) { return fmaxf(a, b); }
-template <> __device__ __forceinline__ double tmin<double>(double a, double b) { return fmin(a, b); }
-template <> __device__ __forceinline__ double tmax<double>(double a, double b) { return fmax(a, b); }
+template <> __device__ __forceinline__ double tmin<double>(double a, double b) { return a < b ? a : b; }
+template <> __device__ __forceinline__ double tmax<double>(double a, double b) { return a > b ? a : b; }
 
 
 // Tuning constants of the warp scheduler inside the kernel.
@@ -325,8 +350,8 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
   // max/min drop the NaN, so dtau = min(cap, r) -- the same limit as flooring alpha.
   const T A = fma(p.dA, p.xi, p.AL);
   const T absA = tabs(A);
-  const T d = Prim<T>::rsqrt(absA + tabs(p.dA * p.u));
-  T dtau = tmax(a.c_abs, (a.c_rel * (absA + tabs(p.u))) * d) * d;
+  const T d = Prim<T>::rsqrt_est(absA + tabs(p.dA * p.u));
+  T dtau = tmax((a.c_rel * (absA + tabs(p.u))) * d, a.c_abs) * d;
   if (DIAG && dtau > p.cap) diag[ST_KAPPA_CAP]++;
   dtau = tmin(tmin(dtau, p.cap), p.r);
 
@@ -337,7 +362,7 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     // Eq. 11: kappa = a' dtau^2/4;  u' = [A dtau + (1+kappa) u] / (1-kappa).
     const T kappa = p.dA * (h * h);
     const T num = fma(A, dtau, fma(kappa, p.u, p.u));
-    u1 = Prim<T>::div(num, T(1) - kappa);
+    u1 = Prim<T>::div_unit(num, T(1) - kappa);
   } else {
     // Picard (A-3): u' <- u; u'' = u + dtau A(xi + dtau (u+u')/4) until
     // |u''-u'| <= tol (|u''| + |A_m| dtau).
