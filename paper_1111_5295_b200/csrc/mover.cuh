@@ -90,6 +90,7 @@ template <> struct Prim<float> {
     float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
   static __device__ __forceinline__ float div(float a, float b) { return a * rcp(b); }
   static __device__ __forceinline__ float rsqrt_est(float x) { return rsqrt(x); }
+  static __device__ __forceinline__ float cap(float c, float absdA) { return c * rsqrt(absdA); }
   static __device__ __forceinline__ float div_unit(float a, float b) { return a * rcp(b); }
 };
 
@@ -108,8 +109,13 @@ template <> struct Prim<double> {
     const double e = fma(-(x * y), y, 1.0);
     return fma(0.5 * y, e, y);
   }
-  // a / b for b in (0, 2) and away from 0 (Eq. 11's denominator 1 - kappa, |kappa| <= kappa_max
-  // < 1 by A-2): MUFU.RCP64H seed + two Newton steps, no special-case path; <= 1.5 ulp.
+  // kappa cap c / sqrt(|dA|) (a step-size bound, like the estimator); |dA| = 0 -> +inf
+  static __device__ __forceinline__ double cap(double c, double absdA) {
+    return absdA > 0.0 ? c * rsqrt_est(absdA) : __longlong_as_double(0x7ff0000000000000LL);
+  }
+  // a / b for a normal, non-zero b (Eq. 11's denominator 1 - kappa in (0, 2) by A-2; the
+  // crossing's u + u_c when moving towards the face): MUFU.RCP64H seed + two Newton steps, no
+  // special-case path; <= 1.5 ulp.  A denormal b gives NaN, which the crossing clamp maps to 0.
   static __device__ __forceinline__ double div_unit(double a, double b) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(b));
@@ -193,7 +199,7 @@ __device__ __forceinline__ void load_cell(const T* __restrict__ sA, T c_cap, Lan
   p.AL = AL;
   p.dA = AR - AL;
   // A-2: dtau <= sqrt(4 kappa_max / |a'|); |dA| = 0 gives +inf (no cap).
-  p.cap = c_cap * Prim<T>::rsqrt(tabs(p.dA));
+  p.cap = Prim<T>::cap(c_cap, tabs(p.dA));
 }
 
 // PER_VISIT a5/O8: flush the stay [xin, xout] in cell c to the block accumulators.
@@ -407,7 +413,7 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     const bool toward = (right ? p.u : -p.u) > T(0);
     T dtc;
     if (toward) {
-      dtc = Prim<T>::div(dxi + dxi, p.u + uc);
+      dtc = Prim<T>::div_unit(dxi + dxi, p.u + uc);   // |u + uc| >= |u| > 0
     } else {
       dtc = (Am == T(0)) ? dtau : Prim<T>::div(uc - p.u, Am);
     }
