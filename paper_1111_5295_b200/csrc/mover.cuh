@@ -446,17 +446,28 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
   }
 }
 
-template <typename T> struct LaunchCfg { static constexpr int min_blocks = 2; };
-template <> struct LaunchCfg<float> { static constexpr int min_blocks = PIC_MINBLOCKS_F32; };
+// Launch shape per precision: fp32 384 threads x 3 blocks/SM (56 registers); fp64 448 threads x
+// 2 blocks/SM (72 registers -> 28 warps/SM instead of 24 with 384-thread blocks).
+#ifndef PIC_BLOCK_F64
+#define PIC_BLOCK_F64 448
+#endif
+template <typename T> struct LaunchCfg {
+  static constexpr int min_blocks = 2;
+  static constexpr int block = PIC_BLOCK_F64;
+};
+template <> struct LaunchCfg<float> {
+  static constexpr int min_blocks = PIC_MINBLOCKS_F32;
+  static constexpr int block = kBlock;
+};
 
 template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2>
-__global__ void __launch_bounds__(kBlock, LaunchCfg<T>::min_blocks)
+__global__ void __launch_bounds__(LaunchCfg<T>::block, LaunchCfg<T>::min_blocks)
 mover_kernel(const MoverArgs<T> a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* sF = reinterpret_cast<double*>(smem_raw);                 // [n] fp64 accumulators
   T* sA = reinterpret_cast<T*>(sF + a.n_cells);                     // [n+2] A on faces + halo
   int32_t* sD = reinterpret_cast<int32_t*>(sA + a.n_cells + 2);     // [n] difference array
-  __shared__ int32_t s_wtot[kBlock / 32];
+  __shared__ int32_t s_wtot[LaunchCfg<T>::block / 32];
 
   // ---- a0: field prologue.  E^{n+1/2} = (E^n + E^{n+1})/2 (north_star; A-11), A = (q/m)E/dx.
   for (int f = threadIdx.x; f < a.n_cells; f += blockDim.x) {

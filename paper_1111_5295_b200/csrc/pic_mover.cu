@@ -46,7 +46,7 @@ cudaError_t set_smem_all(size_t bytes) {
 template <typename T>
 int occupancy(size_t bytes) {
   int nb = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, true, false, false, true>, kBlock, bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, true, false, false, true>, LaunchCfg<T>::block, bytes);
   return nb;
 }
 
@@ -110,7 +110,7 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
   }
   S.last_blocks = S.grid_blocks;
   h->last_kernel = "mover_kernel";
-  dim3 g(S.grid_blocks), b(kBlock);
+  dim3 g(S.grid_blocks), b(LaunchCfg<T>::block);
   with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, [&](auto k) {
     k<<<g, b, h->smem_bytes, h->stream>>>(a);
     return cudaSuccess;
@@ -137,9 +137,10 @@ int mover_configure(pic_handle* h) {
     // persistent grid: one wave of resident blocks (a multiple of the SM count), fewer for
     // small problems so that every warp still gets a few refills' worth of particles.
     const long long full = (long long)h->sm_count * occ;
-    const long long want = (S.n + kBlock * 4 - 1) / (kBlock * 4);
+    const int block = h->elem == 4 ? LaunchCfg<float>::block : LaunchCfg<double>::block;
+    const long long want = (S.n + block * 4 - 1) / (block * 4);
     S.grid_blocks = (int)std::max<long long>(1, std::min(full, want));
-    const long long warps = (long long)S.grid_blocks * (kBlock / 32);
+    const long long warps = (long long)S.grid_blocks * (block / 32);
     long long tile = S.n / (warps * 8);                 // >= 8 claims per warp
 #ifndef PIC_TILE_MAX
 #define PIC_TILE_MAX 512
