@@ -446,10 +446,10 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
   }
 }
 
-// Launch shape per precision: fp32 384 threads x 3 blocks/SM (56 registers); fp64 448 threads x
-// 2 blocks/SM (72 registers -> 28 warps/SM instead of 24 with 384-thread blocks).
+// Launch shape per precision: fp32 384 threads x 3 blocks/SM (56 registers); fp64 512 threads x
+// 2 blocks/SM (64 registers -> 32 warps/SM instead of 24 with 384-thread blocks).
 #ifndef PIC_BLOCK_F64
-#define PIC_BLOCK_F64 448
+#define PIC_BLOCK_F64 512
 #endif
 template <typename T> struct LaunchCfg {
   static constexpr int min_blocks = 2;
