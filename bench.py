@@ -15,6 +15,7 @@ N > 1 (torchrun): independent replicas with different seeds, no data-path collec
 """
 import argparse
 import json
+import math
 import os
 import sys
 import threading
@@ -150,6 +151,9 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1 << 19)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: phase-space cell)")
+    ap.add_argument("--histogram", action="store_true",
+                    help="report the per-particle sub-step / crossing histograms of a step "
+                         "(BASELINE.json configs[3]); keeps 8 B per particle of counters")
     ap.add_argument("--one-per-lane", action="store_true",
                     help="fp32: the one-particle-per-lane kernel instead of the packed two-per-lane one")
     ap.add_argument("--vp", action="store_true",
@@ -187,8 +191,9 @@ def main():
         flags |= B.PIC_FLAG_NO_DEPOSIT
     if args.one_per_lane:
         flags |= B.PIC_FLAG_ONE_PER_LANE
+    init_flags = flags | (B.PIC_FLAG_COUNTS if args.histogram else 0)   # allocates the counters
     pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=args.precision,
-                cn_mode=args.cn_mode, flags=flags, stream=stream)
+                cn_mode=args.cn_mode, flags=init_flags, stream=stream)
     ng = cfg["n_cells"]
     dEn = torch.from_numpy(cfg["E_n"]).cuda()
     dEp = torch.from_numpy(cfg["E_np1"]).cuda()
@@ -206,9 +211,19 @@ def main():
     # ---- one step of the counting build (PIC_FLAG_DIAG) for the exact sub-step / crossing
     # counts of a step (state n is constant, so every step does the same work); the timed steps
     # run the fast build, which does not count per sub-step
-    pic.set_flags(flags | B.PIC_FLAG_DIAG)
+    pic.set_flags(init_flags | B.PIC_FLAG_DIAG)
     pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
     exact = pic.get_stats()
+    hist = None
+    if args.histogram:
+        # 64 bins over [0, 2 x mean) for sub-steps and crossings, last bin = everything above
+        mean = exact["n_sub"] / max(n_p, 1)
+        width = max(1, int(math.ceil(2.0 * mean / 64)))
+        hs, hc = pic.count_histogram(0, width, 65)
+        cum = np.cumsum(hs) / max(int(hs.sum()), 1)
+        pct = {q: int((np.searchsorted(cum, q / 100.0) + 1) * width) for q in (50, 90, 99)}
+        hist = {"bin_width": width, "n_sub": [int(x) for x in hs], "n_cross": [int(x) for x in hc],
+                "n_sub_percentile_upper_bounds": pct}
     pic.set_flags(flags)
 
     # ---- device-resident timing
@@ -300,6 +315,8 @@ def main():
                      "peak_source": "derived: SMs x lanes x 2 x sm_max_mhz (DESIGN.md 6)",
                      "hbm_gbs_algorithmic": n_p * (24 if args.precision == "fp32" else 40) / (k_ms * 1e-3) * 1e-9},
     }
+    if hist is not None:
+        line["substep_histogram"] = hist
     if not args.no_cpu_baseline:
         rate, nsub_s, dts, ns = oracle_rate(cfg, args.cpu_sample)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",

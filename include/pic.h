@@ -146,6 +146,15 @@ int pic_get_particles(pic_handle* h, int species, int which, double* x, double* 
  * (needs PIC_FLAG_COUNTS).  HOST or DEVICE. */
 int pic_get_counts(pic_handle* h, int species, uint32_t* n_sub, uint32_t* n_cross);
 
+/* pic_count_histogram — histograms over the particles of one species of the per-particle sub-step
+ * and crossing counts of the last move (BASELINE.json configs[3]: "sub-step histogram"; needs
+ * PIC_FLAG_COUNTS at pic_init and a move made with it).  Bin k counts the particles with
+ * k*bin_width <= count < (k+1)*bin_width, the last bin everything above; 1 <= n_bins <= 4096.
+ * hist_sub / hist_cross: [n_bins] uint64, HOST or DEVICE, either may be NULL.  Built on the
+ * device (the counts never leave it); synchronises the stream. */
+int pic_count_histogram(pic_handle* h, int species, uint32_t bin_width, int32_t n_bins,
+                        unsigned long long* hist_sub, unsigned long long* hist_cross);
+
 /* pic_get_stats — totals of the last move (synchronises the stream). */
 int pic_get_stats(pic_handle* h, pic_stats* out);
 

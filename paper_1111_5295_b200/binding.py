@@ -27,7 +27,7 @@ PIC_ERR_SUBSTEP_CAP = -4
 EXPORTS = ["pic_init", "pic_move_accumulate", "pic_set_step", "pic_residual", "pic_commit",
            "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_set_flags",
            "pic_kinetic_energy", "pic_rho", "pic_jfnk_step", "pic_jfnk_step_dc",
-           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_last_kernel", "pic_version"]
+           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_last_kernel", "pic_version", "pic_count_histogram"]
 
 
 class PicGrid(C.Structure):
@@ -213,6 +213,12 @@ class Pic:
         n = self.n[species]
         a, b = np.empty(n, np.uint32), np.empty(n, np.uint32)
         self._chk(self._L.pic_get_counts(self._h, C.c_int(species), _ptr(a), _ptr(b)))
+        return a, b
+
+    def count_histogram(self, species=0, bin_width=1, n_bins=256):
+        a, b = np.zeros(n_bins, np.uint64), np.zeros(n_bins, np.uint64)
+        self._chk(self._L.pic_count_histogram(self._h, C.c_int(species), C.c_uint32(bin_width),
+                                              C.c_int32(n_bins), _ptr(a), _ptr(b)))
         return a, b
 
     def get_stats(self):

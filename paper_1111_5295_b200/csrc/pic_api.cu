@@ -110,8 +110,7 @@ int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double*
     const bool pow2 = ng > 1 && (ng & (ng - 1)) == 0;
     const bool two_per_lane = h->elem == 4 && pow2 && h->params.cn_mode == PIC_CN_DIRECT &&
         (size_t)ng * 28 <= 113 * 1024 &&
-        !(h->params.flags & (PIC_FLAG_ONE_PER_LANE | PIC_FLAG_DIAG | PIC_FLAG_COUNTS |
-                             PIC_FLAG_DEPOSIT_PER_VISIT));
+        !(h->params.flags & (PIC_FLAG_ONE_PER_LANE | PIC_FLAG_DEPOSIT_PER_VISIT));
     int32_t nx = two_per_lane ? PIC_NX2 : PIC_NX, nv = 1;
 #ifndef PIC_NVMAX
 #define PIC_NVMAX 1024

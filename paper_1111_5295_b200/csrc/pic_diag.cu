@@ -98,6 +98,37 @@ int pic_get_counts(pic_handle* h, int species, uint32_t* n_sub, uint32_t* n_cros
   return PIC_OK;
 }
 
+int pic_count_histogram(pic_handle* h, int species, uint32_t bin_width, int32_t n_bins,
+                        unsigned long long* hist_sub, unsigned long long* hist_cross) {
+  if (!h) return PIC_ERR_ARG;
+  if (species < 0 || species >= (int)h->sp.size() || bin_width < 1 || n_bins < 1 ||
+      n_bins > kHistMaxBins)
+    return set_err(h, PIC_ERR_ARG, "pic_count_histogram: bad argument");
+  const SpeciesState& S = h->sp[species];
+  if (!S.nsub || !(h->params.flags & PIC_FLAG_COUNTS))
+    return set_err(h, PIC_ERR_STATE, "pic_count_histogram: PIC_FLAG_COUNTS was not set at pic_init");
+  unsigned long long* d = nullptr;
+  const size_t bytes = sizeof(unsigned long long) * (size_t)n_bins;
+  PIC_CUDA(h, cudaMalloc(&d, 2 * bytes));
+  cudaError_t e = cudaMemsetAsync(d, 0, 2 * bytes, h->stream);
+  if (e == cudaSuccess && S.n > 0) {
+    const int blocks = (int)std::min<long long>((S.n + 255) / 256, 4LL * h->sm_count);
+    const size_t sm = sizeof(uint32_t) * (size_t)n_bins;
+    count_hist_kernel<<<blocks, 256, sm, h->stream>>>(S.n, S.nsub, bin_width, n_bins, d);
+    count_hist_kernel<<<blocks, 256, sm, h->stream>>>(S.n, S.ncross, bin_width, n_bins, d + n_bins);
+    h->launches += 2;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess && hist_sub)
+    e = cudaMemcpyAsync(hist_sub, d, bytes, cudaMemcpyDefault, h->stream);
+  if (e == cudaSuccess && hist_cross)
+    e = cudaMemcpyAsync(hist_cross, d + n_bins, bytes, cudaMemcpyDefault, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  cudaFree(d);
+  if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "pic_count_histogram", e);
+  return PIC_OK;
+}
+
 int pic_get_stats(pic_handle* h, pic_stats* out) {
   if (!h || !out) return PIC_ERR_ARG;
   unsigned long long st[ST_COUNT];

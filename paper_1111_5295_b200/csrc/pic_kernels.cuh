@@ -291,4 +291,23 @@ __global__ void rho_kernel(long long n, const T* __restrict__ xi, const int32_t*
   }
 }
 
+// Histogram of per-particle counts (BJ configs[3]: sub-step histogram): bin k holds the particles
+// with k*width <= v < (k+1)*width, the last bin everything above.  Per-block shared-memory
+// histogram (native 32-bit ATOMS), one global 64-bit add per non-empty bin and block.
+constexpr int kHistMaxBins = 4096;
+static __global__ void count_hist_kernel(long long n, const uint32_t* __restrict__ v, uint32_t width,
+                                         int n_bins, unsigned long long* __restrict__ out) {
+  extern __shared__ uint32_t s_h[];
+  for (int b = threadIdx.x; b < n_bins; b += blockDim.x) s_h[b] = 0;
+  __syncthreads();
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const uint32_t b = v[i] / width;
+    atomicAdd(&s_h[b < (uint32_t)n_bins ? b : (uint32_t)n_bins - 1u], 1u);
+  }
+  __syncthreads();
+  for (int b = threadIdx.x; b < n_bins; b += blockDim.x)
+    if (s_h[b]) atomicAdd(&out[b], (unsigned long long)s_h[b]);
+}
+
 }  // namespace picb200

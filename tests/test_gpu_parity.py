@@ -217,6 +217,34 @@ def test_vp_variant_no_deposit(G, oracle, precision):
     vp.close()
 
 
+# ---- device-side sub-step / crossing histograms (BJ configs[3]) against numpy on the counts ----
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_count_histogram(G, precision):
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config3(n=30_011)
+    sp = cfg["species"][0]
+    pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=precision,
+                flags=B.PIC_FLAG_COUNTS | B.PIC_FLAG_VSORT)
+    pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+    ns, nc = pic.get_counts(0)
+    for width, nb in ((1, 4096), (16, 64), (100, 7)):
+        hs, hc = pic.count_histogram(0, width, nb)
+        for h, v in ((hs, ns), (hc, nc)):
+            ref = np.bincount(np.minimum(v // width, nb - 1), minlength=nb)
+            assert np.array_equal(h.astype(np.int64), ref)
+        assert int(hs.sum()) == 30_011
+    st = pic.get_stats()
+    assert int(ns.sum()) == st["n_sub"] and int(nc.sum()) == st["n_cross"]
+    with pytest.raises(B.PicError):
+        pic.count_histogram(0, 0, 16)
+    pic.close()
+    nocount = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=precision)
+    nocount.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+    with pytest.raises(B.PicError):
+        nocount.count_histogram(0, 1, 16)
+    nocount.close()
+
+
 # ---- long orbits: many wraps of the periodic ring (end-point deposit: whole turns) -----------
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_ring_wraps(G, oracle, precision):
