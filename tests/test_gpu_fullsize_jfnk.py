@@ -34,14 +34,25 @@ def test_cfg2_full_size_sampled(oracle):
     pic = B.Pic(ng, cfg["length"], [sp], precision="fp32", cn_mode="direct",
                 flags=B.PIC_FLAG_VSORT | B.PIC_FLAG_COUNTS,
                 stream=torch.cuda.current_stream().cuda_stream)
-    jbar = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], dt)
+    # (a) the counting build: exact per-particle sub-step / crossing counts (flip detection)
+    jbar_c = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], dt)
     st = pic.get_stats()
     assert st["n_substep_cap"] == 0 and st["n_sub"] > 40 * n
     c0, x0, v0 = _device_state(pic, B, torch, B.PIC_STATE_N)
-    c1, x1, v1 = _device_state(pic, B, torch, B.PIC_STATE_NP1)
+    cc, xc, vc = _device_state(pic, B, torch, B.PIC_STATE_NP1)
     nsub = torch.empty(n, dtype=torch.int32, device="cuda")
     ncross = torch.empty(n, dtype=torch.int32, device="cuda")
     pic._chk(pic._L.pic_get_counts(pic._h, C.c_int(0), B._ptr(nsub), B._ptr(ncross)))
+    # (b) the launch configuration bench.py times: the fast build = mover2_kernel (two particles
+    # per lane, packed FP32).  All 1e8 orbits must be bit-identical to the counting build's;
+    # everything below is checked on ITS output.
+    pic.set_flags(B.PIC_FLAG_VSORT)
+    jbar = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], dt)
+    assert pic.last_kernel() == "mover2_kernel"
+    c1, x1, v1 = _device_state(pic, B, torch, B.PIC_STATE_NP1)
+    assert torch.equal(c1, cc) and torch.equal(x1, xc) and torch.equal(v1, vc)
+    assert G.rel_l2(jbar, jbar_c) < 1e-12
+    del cc, xc, vc
     # ---- sampled orbits, one by one through the oracle (particles are independent given E)
     idx = torch.from_numpy(np.sort(np.random.default_rng(3).choice(n, 1 << 16, replace=False))).cuda()
     h = lambda t: t[idx].cpu().numpy()
