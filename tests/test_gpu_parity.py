@@ -123,14 +123,28 @@ def test_fast_build_matches_counting_build(G, precision):
     assert sc["n_sub"] <= sf["n_sub"] < sc["n_sub"] + 4 * 120_007   # grouped upper bound
 
 
+def _tiny_ring(n_cells, n=10_007):
+    """2- or 4-cell ring, dt = 4: every orbit wraps the ring several times (whole-turn deposits)."""
+    length = 0.7 * n_cells
+    xf = W.face_positions(n_cells, length)
+    x = W.uniform01(31, 1, n) * length * (1 - 1e-12)
+    v = 1.5 * W.normal01(31, 2, n)
+    return dict(n_cells=n_cells, length=length, dt=4.0, tol=1e-12,
+                E_n=0.2 * np.sin(2 * math.pi * xf / length),
+                E_np1=0.2 * np.sin(2 * math.pi * xf / length + 0.4),
+                species=[dict(name="e", q_over_m=-1.0, w_q=-length / n, x=x, v=v)])
+
+
+
 # ---- the fast build straight against the oracle: fp32 on power-of-two grids this is
 # mover2_kernel (two particles per lane, packed FP32), fp64 the fast build of mover_kernel
-@pytest.mark.parametrize("case", ["cfg0", "cfg2", "cfg2-vsort", "iaw-2species"])
+@pytest.mark.parametrize("case", ["cfg0", "cfg2", "cfg2-vsort", "iaw-2species", "ring-2-cells"])
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_fast_build_parity_with_oracle(G, oracle, precision, case):
     from paper_1111_5295_b200 import binding as B
     cfg = {"cfg0": lambda: W.config0(), "cfg2": lambda: W.config2(n=100_003),
-           "cfg2-vsort": lambda: W.config2(n=200_003), "iaw-2species": lambda: W.config1(ppc=40)}[case]()
+           "cfg2-vsort": lambda: W.config2(n=200_003), "iaw-2species": lambda: W.config1(ppc=40),
+           "ring-2-cells": lambda: _tiny_ring(2)}[case]()
     extra = B.PIC_FLAG_VSORT if case in ("cfg2-vsort", "iaw-2species") else 0
     m = G.parity(oracle, cfg, precision, extra_flags=extra, fast=True)
     _report(f"fast build {case} {precision} [{m['gpu']['kernel']}]", m)
@@ -141,13 +155,15 @@ def test_fast_build_parity_with_oracle(G, oracle, precision, case):
 
 # ---- the production fp32 kernel (two particles per lane, packed FFMA2/FMUL2/FADD2, mover2.cuh)
 # against the one-particle-per-lane kernel: same arithmetic in the same order => identical orbits
-@pytest.mark.parametrize("case", ["cfg0", "cfg2-vsort", "cfg2-cell", "cfg3-vsort", "cfg2-odd-tail"])
+@pytest.mark.parametrize("case", ["cfg0", "cfg2-vsort", "cfg2-cell", "cfg3-vsort", "cfg2-odd-tail",
+                                  "ring-2-cells", "ring-4-cells-vsort"])
 def test_two_per_lane_matches_one_per_lane(G, case):
     from paper_1111_5295_b200 import binding as B
     cfg = {"cfg0": lambda: W.config0(), "cfg2-vsort": lambda: W.config2(n=150_001),
            "cfg2-cell": lambda: W.config2(n=90_001), "cfg3-vsort": lambda: W.config3(n=20_011),
-           "cfg2-odd-tail": lambda: W.config2(n=65)}[case]()
-    base = 0 if case in ("cfg0", "cfg2-cell") else B.PIC_FLAG_VSORT
+           "cfg2-odd-tail": lambda: W.config2(n=65), "ring-2-cells": lambda: _tiny_ring(2),
+           "ring-4-cells-vsort": lambda: _tiny_ring(4)}[case]()
+    base = 0 if case in ("cfg0", "cfg2-cell", "ring-2-cells") else B.PIC_FLAG_VSORT
     sp = cfg["species"][0]
     out = {}
     for name, flags in (("two", base), ("one", base | B.PIC_FLAG_ONE_PER_LANE)):
