@@ -128,11 +128,15 @@ template <> struct Prim<double> {
 };
 
 // xi in [0,1] (inclusive, A-5).  fp32: one unsigned compare of the bit pattern (non-negative
-// floats order like their bits; a set sign bit or a NaN compares above 1.0f's pattern).
+// floats order like their bits; a set sign bit or a NaN compares above 1.0f's pattern; -0.0 is
+// rejected and then takes a zero-length crossing, A-5).
 template <typename T> __device__ __forceinline__ bool in_unit(T x);
 template <> __device__ __forceinline__ bool in_unit<float>(float x) {
   return __float_as_uint(x) <= 0x3f800000u; }
-template <> __device__ __forceinline__ bool in_unit<double>(double x) { return x >= 0.0 && x <= 1.0; }
+// fp64: the same test on the 64-bit pattern (two integer compares on the ALU pipe instead of two
+// DSETP on the FP64 pipe, which bounds the fp64 kernel)
+template <> __device__ __forceinline__ bool in_unit<double>(double x) {
+  return (unsigned long long)__double_as_longlong(x) <= 0x3ff0000000000000ull; }
 
 template <typename T> __device__ __forceinline__ T tabs(T x);
 template <> __device__ __forceinline__ float tabs<float>(float x) { return fabsf(x); }
