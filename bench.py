@@ -151,6 +151,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1 << 19)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: phase-space cell)")
+    ap.add_argument("--microbench", action="store_true",
+                    help="only run the P:86 instruction micro-benchmarks (pic_microbench) and print them")
     ap.add_argument("--histogram", action="store_true",
                     help="report the per-particle sub-step / crossing histograms of a step "
                          "(BASELINE.json configs[3]); keeps 8 B per particle of counters")
@@ -179,6 +181,19 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     B.load()
+    if args.microbench:
+        if rank == 0:
+            try:
+                mhz = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("sm_max_mhz") or 1965.0)
+            except Exception:  # noqa: BLE001
+                mhz = 1965.0
+            sampler = ClockSampler(local_rank)
+            sampler.start()
+            mb = B.microbench(iters=200000, sm_mhz=mhz)
+            print(json.dumps({"microbench": mb, "sm_mhz_for_per_clk": mhz, "clocks": sampler.stop(),
+                              "fp32_gflops_measured_ffma": 2 * mb["ffma"]["thread_gops"],
+                              "fp64_gflops_measured_dfma": 2 * mb["dfma"]["thread_gops"]}), flush=True)
+        return
 
     # replicas only: every rank runs its own copy of the workload with its own seed
     from paper_1111_5295_b200 import replicas as _rep

@@ -219,6 +219,15 @@ const char* pic_last_error(const pic_handle* h);
  * (fp32, two particles per lane, packed FP32; csrc/mover2.cuh) or "mover_kernel" (csrc/mover.cuh);
  * "" before the first move.  For bench lines and profiles. */
 const char* pic_last_kernel(const pic_handle* h);
+/* pic_microbench — the paper's micro-benchmark method on the current device: peak rate
+ * of one instruction class in 1e9 thread-operations per second over the whole chip, from a
+ * full-occupancy kernel of independent dependent chains timed with CUDA events (divide by n_sm
+ * and the SM clock for operations per clock and SM).  which: 0 FFMA, 1 FFMA2 (packed; counts two
+ * per thread), 2 FMNMX (ALU pipe), 3 MUFU.RSQ, 4 DFMA, 5 the mix 4 FFMA2 + 4 FMNMX per iteration.
+ * iters: loop length (e.g. 20000).  n_sm may be NULL.  Needs no handle; runs on the default
+ * stream and synchronises it. */
+int pic_microbench(int which, int iters, double* thread_gops, int* n_sm);
+
 /* Library/device identification for logs: fills buf with e.g. "pic_b200 sm_100a ...". */
 int pic_version(char* buf, int buflen);
 

@@ -27,7 +27,7 @@ PIC_ERR_SUBSTEP_CAP = -4
 EXPORTS = ["pic_init", "pic_move_accumulate", "pic_set_step", "pic_residual", "pic_commit",
            "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_set_flags",
            "pic_kinetic_energy", "pic_rho", "pic_jfnk_step", "pic_jfnk_step_dc",
-           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_last_kernel", "pic_version", "pic_count_histogram"]
+           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_last_kernel", "pic_version", "pic_count_histogram", "pic_microbench"]
 
 
 class PicGrid(C.Structure):
@@ -122,6 +122,24 @@ def _check_f64(a, n, name):
         ok, size = a.dtype == torch.float64, a.numel()
     if not ok or size != n:
         raise ValueError(f"{name}: need float64[{n}]")
+
+
+MICROBENCH = {0: "ffma", 1: "ffma2", 2: "fmnmx", 3: "mufu_rsq", 4: "dfma", 5: "ffma2+fmnmx"}
+
+
+def microbench(iters=20000, sm_mhz=1965.0):
+    """P:86 micro-benchmarks: 1e9 thread-operations per second per instruction class, and the
+    same per clock and SM at `sm_mhz`."""
+    L = load()
+    out = {}
+    for which, name in MICROBENCH.items():
+        gops, sms = C.c_double(0.0), C.c_int(0)
+        rc = L.pic_microbench(C.c_int(which), C.c_int(iters), C.byref(gops), C.byref(sms))
+        if rc != 0:
+            raise PicError(rc, "pic_microbench")
+        out[name] = {"thread_gops": gops.value,
+                     "per_clk_per_sm": gops.value * 1e3 / (sms.value * sm_mhz)}
+    return out
 
 
 def version():
