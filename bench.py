@@ -151,6 +151,9 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1 << 19)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: phase-space cell)")
+    ap.add_argument("--fp64-n", type=int, default=20_000_000,
+                    help="with --precision fp32: also time the fp64 mover on the first N particles of "
+                         "the same workload and report it under 'fp64' (0 = skip)")
     ap.add_argument("--microbench", action="store_true",
                     help="only run the P:86 instruction micro-benchmarks (pic_microbench) and print them")
     ap.add_argument("--histogram", action="store_true",
@@ -332,13 +335,39 @@ def main():
     }
     if hist is not None:
         line["substep_histogram"] = hist
+    pic.close()
+    pic = None
+    # ---- BASELINE.json's metric names both precisions: the fp64 instantiation of the mover on
+    # the first fp64_n particles of the same workload (same fields, same dt), kernel-timed
+    if args.precision == "fp32" and args.fp64_n > 0 and not args.vp:
+        n64 = min(args.fp64_n, n_p)
+        sp64 = dict(sp, x=sp["x"][:n64], v=sp["v"][:n64], w_q=sp["w_q"] * n_p / n64)
+        p64 = B.Pic(cfg["n_cells"], cfg["length"], [sp64], precision="fp64", cn_mode=args.cn_mode,
+                    flags=(0 if args.no_vsort else B.PIC_FLAG_VSORT) | B.PIC_FLAG_DIAG, stream=stream)
+        p64.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+        ex64 = p64.get_stats()
+        p64.set_flags(0 if args.no_vsort else B.PIC_FLAG_VSORT)
+        for _ in range(3):
+            p64.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+        k64 = []
+        for _ in range(5):
+            p64.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+            k64.append(p64.get_stats()["last_move_ms"])
+        k64 = float(np.mean(k64))
+        ops64 = OPS_INCELL * (ex64["n_sub"] - ex64["n_cross"]) + OPS_CROSS * ex64["n_cross"]
+        peak64 = sms * 64 * 2 * sm_max_mhz * 1e-3
+        line["fp64"] = {"value": ex64["n_sub"] / (k64 * 1e-3), "unit": UNIT, "n_particles": n64,
+                        "kernel": p64.last_kernel(), "kernel_ms": k64,
+                        "roofline": {"bound": "alu", "achieved": ops64 / (k64 * 1e-3) * 1e-9,
+                                     "peak": peak64, "unit": "GOp/s",
+                                     "frac": ops64 / (k64 * 1e-3) * 1e-9 / peak64}}
+        p64.close()
     if not args.no_cpu_baseline:
         rate, nsub_s, dts, ns = oracle_rate(cfg, args.cpu_sample)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"first {ns} particles of {args.workload} "
                                           f"({nsub_s} sub-steps, {dts:.1f} s), serial fp64 oracle"}
     print(json.dumps(line), flush=True)
-    pic.close()
     if world > 1:
         dist.destroy_process_group()
 
