@@ -16,8 +16,8 @@
 // the warp now re-queues 64 slots instead of 32 lanes.
 //
 // Per-cell constants {A_L, dA, kappa cap} are precomputed once per block into a float4 table
-// (three loads on cell entry instead of two loads + FADD + MUFU.RSQ + FMUL): 28 B of shared memory per cell,
-// two 384-thread blocks per SM (<= 85 registers per thread).
+// (three loads on cell entry instead of two loads + FADD + MUFU.RSQ + FMUL): 28 B of shared memory
+// per cell, two 512-thread blocks per SM (64 registers per thread, 32 warps = 2,048 orbits per SM).
 #pragma once
 #include "mover.cuh"
 
