@@ -327,7 +327,8 @@ int pic_move_accumulate(pic_handle* h, const double* E_n, const double* E_np1, d
   }
   PIC_CUDA(h, cudaEventRecord(h->ev1, h->stream));
   const int32_t ng = h->grid.n_cells;
-  reduce_rows_kernel<<<(ng + 127) / 128, 128, 0, h->stream>>>(row, ng, h->d_partial, h->d_jbar);
+  reduce_rows_kernel<<<(ng + kRedCols - 1) / kRedCols, dim3(kRedCols, kRedRows), 0, h->stream>>>(
+      row, ng, h->d_partial, h->d_jbar);
   h->launches++;
   PIC_CUDA(h, cudaGetLastError());
   h->have_np1 = !(h->params.flags & PIC_FLAG_NO_STORE);

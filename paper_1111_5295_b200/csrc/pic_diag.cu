@@ -185,6 +185,12 @@ int pic_kinetic_energy(pic_handle* h, int which, double* ke_out) {
   return PIC_OK;
 }
 
+// one thread per kRhoChunk consecutive particles
+static int rho_grid(long long n) {
+  const long long threads = (n + kRhoChunk - 1) / kRhoChunk;
+  return (int)std::max<long long>(1, (threads + 255) / 256);
+}
+
 int pic_rho(pic_handle* h, int which, double* rho_out) {
   if (!h || !rho_out) return PIC_ERR_ARG;
   if (which == PIC_STATE_NP1 && !h->have_np1)
@@ -196,10 +202,10 @@ int pic_rho(pic_handle* h, int which, double* rho_out) {
   for (auto& S : h->sp) {
     if (S.n == 0) continue;
     if (h->elem == 4)
-      rho_kernel<float><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, (const float*)S.xi[b], S.cell[b],
+      rho_kernel<float><<<rho_grid(S.n), 256, 0, h->stream>>>(S.n, (const float*)S.xi[b], S.cell[b],
                                                               ng, S.w_q / dx, h->d_resid);
     else
-      rho_kernel<double><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, (const double*)S.xi[b],
+      rho_kernel<double><<<rho_grid(S.n), 256, 0, h->stream>>>(S.n, (const double*)S.xi[b],
                                                                S.cell[b], ng, S.w_q / dx, h->d_resid);
     h->launches++;
   }

@@ -186,14 +186,28 @@ __global__ void scatter_kernel(long long n, const int32_t* __restrict__ cell_in,
   }
 }
 
-// a8: jbar_f = sum over block rows (fixed order -> reproducible given the rows).
-static __global__ void reduce_rows_kernel(int rows, int32_t n_cells, const double* __restrict__ partial,
-                                   double* __restrict__ jbar) {
-  const int f = blockIdx.x * blockDim.x + threadIdx.x;
-  if (f >= n_cells) return;
+// a8: jbar_f = sum over block rows (fixed order -> reproducible given the rows).  A block of
+// kRedCols x kRedRows threads owns kRedCols faces: thread (c, r) adds rows r, r + kRedRows, ...
+// of its face (coalesced across c), then the kRedRows partial sums are added in order.  (One
+// thread per face looping over all rows was latency-bound: 64 us for 592 rows x 512 faces.)
+constexpr int kRedCols = 32, kRedRows = 16;
+static __global__ void __launch_bounds__(kRedCols * kRedRows)
+reduce_rows_kernel(int rows, int32_t n_cells, const double* __restrict__ partial,
+                   double* __restrict__ jbar) {
+  __shared__ double sm[kRedRows][kRedCols + 1];
+  const int c = threadIdx.x, r0 = threadIdx.y;
+  const int f = blockIdx.x * kRedCols + c;
   double s = 0.0;
-  for (int r = 0; r < rows; ++r) s += partial[(size_t)r * n_cells + f];
-  jbar[f] = s;
+  if (f < n_cells)
+    for (int r = r0; r < rows; r += kRedRows) s += partial[(size_t)r * n_cells + f];
+  sm[r0][c] = s;
+  __syncthreads();
+  if (r0 == 0 && f < n_cells) {
+    double t = 0.0;
+#pragma unroll
+    for (int k = 0; k < kRedRows; ++k) t += sm[k][c];
+    jbar[f] = t;
+  }
 }
 
 // a9: R_f = (E^{n+1}_f - E^n_f)/dt + jbar_f - <jbar>  (eps0 = 1).  One block.
@@ -275,19 +289,50 @@ __global__ void sumsq_kernel(long long n, const T* __restrict__ v, double* __res
 }
 
 // rho on cell centres, quadratic B-spline (A-10): with p = xi in [0,1] inside cell c the
-// weights on cells c-1, c, c+1 are (1-p)^2/2, 3/4 - (p-1/2)^2, p^2/2.
+// weights on cells c-1, c, c+1 are (1-p)^2/2, 3/4 - (p-1/2)^2, p^2/2.  The state is binned by
+// cell, so every thread takes kRhoChunk CONSECUTIVE particles and keeps the three sums of the
+// current cell in registers; they go to memory when the cell changes and at the end of the
+// chunk, there summed over the warp first when all its lanes are in the same cell (one fp64
+// atomic per warp and cell instead of one per particle: 1.1 ms -> tens of us at 2e6 particles).
+constexpr int kRhoChunk = 32;
+__device__ __forceinline__ void rho_flush(double* __restrict__ rho, int32_t n_cells, int32_t c,
+                                          double wl, double wc, double wr) {
+  atomicAdd(&rho[c == 0 ? n_cells - 1 : c - 1], wl);
+  atomicAdd(&rho[c], wc);
+  atomicAdd(&rho[c + 1 == n_cells ? 0 : c + 1], wr);
+}
 template <typename T>
 __global__ void rho_kernel(long long n, const T* __restrict__ xi, const int32_t* __restrict__ cell,
                            int32_t n_cells, double w_over_dx, double* __restrict__ rho) {
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
-       i += (long long)gridDim.x * blockDim.x) {
-    const double p = (double)xi[i];
+  const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  const long long i0 = t * kRhoChunk, i1 = i0 + kRhoChunk < n ? i0 + kRhoChunk : n;
+  int32_t cur = -1;
+  double wl = 0.0, wc = 0.0, wr = 0.0;
+  for (long long i = i0; i < i1; ++i) {
     const int32_t c = cell[i];
-    const int32_t cl = c == 0 ? n_cells - 1 : c - 1;
-    const int32_t cr = c + 1 == n_cells ? 0 : c + 1;
-    atomicAdd(&rho[cl], w_over_dx * 0.5 * (1.0 - p) * (1.0 - p));
-    atomicAdd(&rho[c], w_over_dx * (0.75 - (p - 0.5) * (p - 0.5)));
-    atomicAdd(&rho[cr], w_over_dx * 0.5 * p * p);
+    if (c != cur) {
+      if (cur >= 0) rho_flush(rho, n_cells, cur, wl, wc, wr);
+      cur = c;
+      wl = wc = wr = 0.0;
+    }
+    const double p = (double)xi[i];
+    wl += w_over_dx * 0.5 * (1.0 - p) * (1.0 - p);
+    wc += w_over_dx * (0.75 - (p - 0.5) * (p - 0.5));
+    wr += w_over_dx * 0.5 * p * p;
+  }
+  // the whole warp reaches this point (the chunk loop is the only divergent part)
+  const unsigned full = 0xffffffffu;
+  const int32_t c0 = __shfl_sync(full, cur, 0);
+  if (__all_sync(full, cur == c0 && cur >= 0)) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      wl += __shfl_xor_sync(full, wl, o);
+      wc += __shfl_xor_sync(full, wc, o);
+      wr += __shfl_xor_sync(full, wr, o);
+    }
+    if ((threadIdx.x & 31) == 0) rho_flush(rho, n_cells, cur, wl, wc, wr);
+  } else if (cur >= 0) {
+    rho_flush(rho, n_cells, cur, wl, wc, wr);
   }
 }
 
