@@ -185,10 +185,10 @@ int pic_kinetic_energy(pic_handle* h, int which, double* ke_out) {
   return PIC_OK;
 }
 
-// one thread per kRhoChunk consecutive particles
-static int rho_grid(long long n) {
-  const long long threads = (n + kRhoChunk - 1) / kRhoChunk;
-  return (int)std::max<long long>(1, (threads + 255) / 256);
+// persistent grid: a few blocks per SM, fewer for small species (>= one full pass per block)
+static int rho_grid(const pic_handle* h, long long n) {
+  const long long want = (n + 512LL * kRhoChunk - 1) / (512LL * kRhoChunk);
+  return (int)std::max<long long>(1, std::min<long long>(want, 4LL * h->sm_count));
 }
 
 int pic_rho(pic_handle* h, int which, double* rho_out) {
@@ -199,13 +199,18 @@ int pic_rho(pic_handle* h, int which, double* rho_out) {
   const double dx = h->grid.length / ng;
   const int b = which == PIC_STATE_N ? h->cur : 1 - h->cur;
   PIC_CUDA(h, cudaMemsetAsync(h->d_resid, 0, sizeof(double) * ng, h->stream));
+  const size_t rho_smem = sizeof(double) * (size_t)ng;
+  if (rho_smem > 48 * 1024) {
+    PIC_CUDA(h, cudaFuncSetAttribute(rho_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rho_smem));
+    PIC_CUDA(h, cudaFuncSetAttribute(rho_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rho_smem));
+  }
   for (auto& S : h->sp) {
     if (S.n == 0) continue;
     if (h->elem == 4)
-      rho_kernel<float><<<rho_grid(S.n), 256, 0, h->stream>>>(S.n, (const float*)S.xi[b], S.cell[b],
+      rho_kernel<float><<<rho_grid(h, S.n), 512, rho_smem, h->stream>>>(S.n, (const float*)S.xi[b], S.cell[b],
                                                               ng, S.w_q / dx, h->d_resid);
     else
-      rho_kernel<double><<<rho_grid(S.n), 256, 0, h->stream>>>(S.n, (const double*)S.xi[b],
+      rho_kernel<double><<<rho_grid(h, S.n), 512, rho_smem, h->stream>>>(S.n, (const double*)S.xi[b],
                                                                S.cell[b], ng, S.w_q / dx, h->d_resid);
     h->launches++;
   }

@@ -292,8 +292,9 @@ __global__ void sumsq_kernel(long long n, const T* __restrict__ v, double* __res
 // weights on cells c-1, c, c+1 are (1-p)^2/2, 3/4 - (p-1/2)^2, p^2/2.  The state is binned by
 // cell, so every thread takes kRhoChunk CONSECUTIVE particles and keeps the three sums of the
 // current cell in registers; they go to memory when the cell changes and at the end of the
-// chunk, there summed over the warp first when all its lanes are in the same cell (one fp64
-// atomic per warp and cell instead of one per particle: 1.1 ms -> tens of us at 2e6 particles).
+// chunk, there summed over the warp first when all its lanes are in the same cell, into the
+// block's shared-memory copy of rho (global fp64 atomics per particle took 1.1 ms at 2e6
+// particles).
 constexpr int kRhoChunk = 32;
 __device__ __forceinline__ void rho_flush(double* __restrict__ rho, int32_t n_cells, int32_t c,
                                           double wl, double wc, double wr) {
@@ -301,39 +302,53 @@ __device__ __forceinline__ void rho_flush(double* __restrict__ rho, int32_t n_ce
   atomicAdd(&rho[c], wc);
   atomicAdd(&rho[c + 1 == n_cells ? 0 : c + 1], wr);
 }
+// Persistent blocks: each owns one contiguous span of the particle list and a shared-memory copy
+// of rho (dynamic, n_cells doubles), flushed to global memory once at the end.
 template <typename T>
 __global__ void rho_kernel(long long n, const T* __restrict__ xi, const int32_t* __restrict__ cell,
                            int32_t n_cells, double w_over_dx, double* __restrict__ rho) {
-  const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  const long long i0 = t * kRhoChunk, i1 = i0 + kRhoChunk < n ? i0 + kRhoChunk : n;
-  int32_t cur = -1;
-  double wl = 0.0, wc = 0.0, wr = 0.0;
-  for (long long i = i0; i < i1; ++i) {
-    const int32_t c = cell[i];
-    if (c != cur) {
-      if (cur >= 0) rho_flush(rho, n_cells, cur, wl, wc, wr);
-      cur = c;
-      wl = wc = wr = 0.0;
-    }
-    const double p = (double)xi[i];
-    wl += w_over_dx * 0.5 * (1.0 - p) * (1.0 - p);
-    wc += w_over_dx * (0.75 - (p - 0.5) * (p - 0.5));
-    wr += w_over_dx * 0.5 * p * p;
-  }
-  // the whole warp reaches this point (the chunk loop is the only divergent part)
+  extern __shared__ double s_rho[];
+  for (int f = threadIdx.x; f < n_cells; f += blockDim.x) s_rho[f] = 0.0;
+  __syncthreads();
+  const long long stride = (long long)blockDim.x * kRhoChunk;
+  const long long per_block = ((n + gridDim.x - 1) / gridDim.x + stride - 1) / stride * stride;
+  const long long b0 = blockIdx.x * per_block;
+  const long long b1 = b0 + per_block < n ? b0 + per_block : n;
   const unsigned full = 0xffffffffu;
-  const int32_t c0 = __shfl_sync(full, cur, 0);
-  if (__all_sync(full, cur == c0 && cur >= 0)) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      wl += __shfl_xor_sync(full, wl, o);
-      wc += __shfl_xor_sync(full, wc, o);
-      wr += __shfl_xor_sync(full, wr, o);
+  // the trip count is the same for every thread of the block (a lane past the end has an empty run)
+  for (long long base = b0; base < b1; base += stride) {
+    const long long i0 = base + (long long)threadIdx.x * kRhoChunk;
+    const long long i1 = i0 + kRhoChunk < b1 ? i0 + kRhoChunk : b1;
+    int32_t cur = -1;
+    double wl = 0.0, wc = 0.0, wr = 0.0;
+    for (long long i = i0; i < i1; ++i) {
+      const int32_t c = cell[i];
+      if (c != cur) {
+        if (cur >= 0) rho_flush(s_rho, n_cells, cur, wl, wc, wr);
+        cur = c;
+        wl = wc = wr = 0.0;
+      }
+      const double p = (double)xi[i];
+      wl += w_over_dx * 0.5 * (1.0 - p) * (1.0 - p);
+      wc += w_over_dx * (0.75 - (p - 0.5) * (p - 0.5));
+      wr += w_over_dx * 0.5 * p * p;
     }
-    if ((threadIdx.x & 31) == 0) rho_flush(rho, n_cells, cur, wl, wc, wr);
-  } else if (cur >= 0) {
-    rho_flush(rho, n_cells, cur, wl, wc, wr);
+    const int32_t c0 = __shfl_sync(full, cur, 0);
+    if (__all_sync(full, cur == c0 && cur >= 0)) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        wl += __shfl_xor_sync(full, wl, o);
+        wc += __shfl_xor_sync(full, wc, o);
+        wr += __shfl_xor_sync(full, wr, o);
+      }
+      if ((threadIdx.x & 31) == 0) rho_flush(s_rho, n_cells, cur, wl, wc, wr);
+    } else if (cur >= 0) {
+      rho_flush(s_rho, n_cells, cur, wl, wc, wr);
+    }
   }
+  __syncthreads();
+  for (int f = threadIdx.x; f < n_cells; f += blockDim.x)
+    if (s_rho[f] != 0.0) atomicAdd(&rho[f], s_rho[f]);
 }
 
 // Histogram of per-particle counts (BJ configs[3]: sub-step histogram): bin k holds the particles
