@@ -14,10 +14,16 @@
 // P-3 Eq. 11 == Picard fixed point, P-4 estimator bound, P-5 crossing invariants +
 // bisection, P-6 per-cell discrete continuity, P-7 endpoint formula, P-8 mean current,
 // P-9 energy identity, P-10 refinement to the harmonic oscillator / RK reference,
-// P-11 hand-stepped tiny cases, P-12 residual sum.
-// Parity unpinned (self-consistency only; the paper is silent): kappa_max cap (A-2),
-// the exact form of the Picard convergence test (A-3), the face convention (A-5),
-// the sub-step cap (A-9), the face/cell index convention.
+// P-11 hand-stepped tiny cases, P-12 residual sum; oracle_bin against hand values and the
+// identity cell*dx + s = x; and pins on workloads that EXECUTE the guard branches: the A-2
+// kappa cap (binding on most sub-steps), the O7 discriminant and crossing-time clamps
+// (rounding coincidences: particles that end a step exactly on a face), the A-3 Picard cap
+// (picard_max = 1 is the explicit midpoint rule) -- each checked against what the mathematics
+// still fixes there (1 - kappa >= 1/2, sum dtau = dt, closed-form end state, P-5, P-6, P-9).
+// Parity unpinned (self-consistency only; the paper is silent on the CHOICE, the code that
+// implements it is pinned as above): the value kappa_max = 0.5 (A-2), the exact form of the
+// Picard convergence test (A-3), the face convention (A-5), the sub-step cap (A-9), the
+// face/cell index convention.
 //
 // Conventions (SURVEY 8 "Common notation"): periodic [0,L), n_cells uniform cells,
 // dx = L/n_cells; face f at x_f = f*dx; cell c spans faces c and (c+1) mod n_cells.

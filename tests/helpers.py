@@ -54,3 +54,58 @@ def continuity_residual(o, cfg, start, end, jbar):
         o.rho(n_cells, length, sp["w_q"], c1, s1, rho1)
     div = dt * (np.roll(jbar, -1) - jbar) / dx
     return rho1 - rho0 + div, div
+
+
+# ---- workloads that EXECUTE the guard branches of the mover ----------
+# Input design only (kinematics of a uniformly accelerated particle); no arithmetic of the method.
+def kappa_cap_cfg(n=4000, seed=9):
+    """Strong, short-wavelength field and slow particles: with loose estimator tolerances the
+    A-2 cap dtau <= sqrt(4 kappa_max/|a'|) binds on most sub-steps (a' of both signs)."""
+    import math
+    from paper_1111_5295_b200 import workloads as W
+    n_cells, length = 16, 8.0
+    xf = W.face_positions(n_cells, length)
+    E = 3.0 * np.sin(2 * math.pi * xf / length) + 2.0 * np.cos(6 * math.pi * xf / length)
+    x = W.uniform01(seed, 1, n) * length * (1 - 1e-12)
+    v = 0.3 * W.normal01(seed, 2, n)
+    return dict(n_cells=n_cells, length=length, dt=6.0, tol=1e-12, E_n=E, E_np1=0.8 * E,
+                species=[dict(name="e", q_over_m=-1.0, w_q=-length / n, x=x, v=v)])
+
+
+LOOSE = dict(eps_a=1.0, eps_r=0.9)      # estimator tolerances under which the cap binds
+
+
+def landing_cfg(kind, n_cells=4096, dt=1.0, seed=3, q_over_m=-1.0):
+    """Rounding-coincidence workload for the crossing guards (O7: D < 0 clamp, dtau_c clamp).
+    dx = 1.  Every even cell c carries a UNIFORM field (faces c and c+1 equal) and one particle
+    that moves towards its right (c % 4 == 0) or left (c % 4 == 2) face at distance `dist`, with
+    the field chosen so that in exact arithmetic it is exactly ON that face at t = dt:
+      kind 'land': arrives with a random non-zero velocity (a = 2 (dist - v0 dt)/dt^2);
+      kind 'turn': arrives with v = 0, the apex of its parabola (v0 = 2 dist/dt, a = -v0/dt).
+    With estimator tolerances eps_a = eps_r = 1 the whole dt is ONE tentative sub-step, which
+    lands within an ulp or two of the face: about half the particles overshoot it and take the
+    crossing branch with a discriminant / crossing time within rounding of its bound.
+    `dist` is a multiple of 2^-30 so that x = cell + s is exact in fp64 (and xi in the kernel).
+    Returns (cfg, state, closed_form) with closed_form = (X1 unwrapped, v1)."""
+    rng = np.random.default_rng(seed)
+    m = n_cells // 2
+    sgn = np.where(np.arange(m) % 2 == 0, 1.0, -1.0)
+    dist = np.round(rng.uniform(0.1, 0.9, m) * 2.0 ** 30) / 2.0 ** 30
+    if kind == "turn":
+        v0 = 2.0 * dist / dt
+        a = -v0 / dt
+    else:
+        v0 = rng.uniform(0.2, 1.5, m) * dist / dt
+        a = 2.0 * (dist - v0 * dt) / dt ** 2
+    v0, a = sgn * v0, sgn * a
+    E = np.zeros(n_cells)
+    E[0::2] = a / q_over_m
+    E[1::2] = a / q_over_m
+    cells = np.arange(0, n_cells, 2).astype(np.int32)
+    s0 = np.where(sgn > 0, 1.0 - dist, dist)
+    x = cells + s0
+    assert np.array_equal(x - cells, s0)
+    cfg = dict(n_cells=n_cells, length=float(n_cells), dt=dt, tol=1e-12, E_n=E, E_np1=E.copy(),
+               species=[dict(name="e", q_over_m=q_over_m, w_q=-float(n_cells) / m, x=x, v=v0)])
+    X1 = cells + np.where(sgn > 0, 1.0, 0.0)
+    return cfg, [(cells, s0, v0)], (X1, v0 + a * dt)

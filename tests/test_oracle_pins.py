@@ -7,7 +7,8 @@ import numpy as np
 import pytest
 
 from paper_1111_5295_b200 import workloads as W
-from helpers import continuity_residual, oracle_run, unwrapped
+from helpers import (LOOSE, continuity_residual, kappa_cap_cfg, landing_cfg, oracle_run,
+                     unwrapped)
 
 
 def _cfg(n_cells, length, x, v, E_n, E_np1, dt, q_over_m=-1.0, w_q=None):
@@ -34,7 +35,8 @@ def test_p1_free_streaming(oracle, mode):
     X0, X1 = unwrapped(cfg, r)
     assert np.max(np.abs(X1 - (X0 + v * dt))) < 5e-14
     assert np.array_equal(r["v"], v)
-    assert np.all(r["n_sub"] == r["n_cross"] + 1) or np.all(r["n_sub"] >= r["n_cross"])
+    # E = 0: alpha = 0, so dtau = r (A-1): every sub-step but the last one is a crossing
+    assert np.all(r["n_sub"] == r["n_cross"] + 1)
     # every crossing was counted: k = floor(X1/dx) - cell0 up to face landings
     assert np.all(np.abs(r["k"] - (np.floor(X1 / (length / n_cells)) - r["cell0"])) <= 1)
 
@@ -337,3 +339,176 @@ def test_workload_shape_cfg0(oracle):
     st = out["stats"]
     assert 5.5 < st.n_sub / 6400 < 6.8 and 0.55 < st.n_cross / st.n_sub < 0.75
     assert st.n_kappa_cap == st.n_substep_cap == st.n_neg_disc == st.n_picard_cap == 0
+
+
+# ---- oracle_bin (x -> cell, s): the start state of every other pin ------------------------------
+def test_oracle_bin(oracle):
+    """cell*dx + s == x to rounding, 0 <= s <= dx, cell in range; exact hand values on a grid
+    whose dx is a power of two; the edges x = 0, a face, nextafter(L, 0)."""
+    n_cells, length = 8, 4.0                       # dx = 0.5: everything below is exact
+    x = np.array([0.0, 0.5, 1.25, 3.5, np.nextafter(4.0, 0.0), 0.4999999999999999, 2.0])
+    cell, s = oracle.bin_particles(n_cells, length, x)
+    assert cell.tolist() == [0, 1, 2, 7, 7, 0, 4]
+    assert s.tolist() == [0.0, 0.0, 0.25, 0.0, np.nextafter(4.0, 0.0) - 3.5, 0.4999999999999999, 0.0]
+    # a grid whose dx is not representable: the identity and the bounds, to rounding
+    n_cells, length = 4096, 4096 * (100.0 * math.pi / 256.0)
+    dx = length / n_cells
+    rng = np.random.default_rng(4)
+    x = np.concatenate([rng.uniform(0, length, 20000), np.arange(n_cells) * dx,
+                        np.nextafter(np.arange(1, n_cells + 1) * dx, 0.0), [0.0]])
+    x = np.minimum(x, np.nextafter(length, 0.0))
+    cell, s = oracle.bin_particles(n_cells, length, x)
+    assert cell.min() >= 0 and cell.max() <= n_cells - 1
+    assert s.min() >= 0.0 and s.max() <= dx
+    assert np.max(np.abs(cell * dx + s - x)) <= 2 * np.spacing(length)
+    # a plausible slip (cell = round or ceil, s measured from the wrong face) moves s by ~dx
+    frac = x / dx - np.floor(x / dx)
+    assert np.max(np.abs(s / dx - frac)) < 1e-9
+    # x on a face may bin into either neighbour (A-5: s = 0 or s = dx), never elsewhere
+    faces = np.arange(n_cells) * dx
+    c2, s2 = oracle.bin_particles(n_cells, length, faces)
+    ok = ((c2 == np.arange(n_cells)) & (s2 < 1e-9)) | ((c2 == np.arange(n_cells) - 1) & (dx - s2 < 1e-9))
+    assert ok.all()
+
+
+# ---- guard branches (SURVEY A-2, A-3, O7): workloads on which they EXECUTE, checked against
+# what the mathematics still fixes when they do -------------------------------------------------
+def test_guard_kappa_cap_binds(oracle):
+    """A-2: dtau <= sqrt(4 kappa_max/|a'|).  With loose estimator tolerances the cap binds on
+    most sub-steps; then 1 - kappa stays in [0.5, 1.5] (Eq. 11's denominator), every
+    orbit still uses up exactly dt, the crossing solve keeps a real root in (0, dtau] (no
+    discriminant or crossing-time clamp), and continuity (P-6) and the energy identity (P-9)
+    hold to rounding -- they do not depend on the step sizes."""
+    cfg = kappa_cap_cfg()
+    for mode in (oracle.PICARD, oracle.DIRECT):
+        p = oracle.make_params(cn_mode=mode, tol=1e-14, **LOOSE)
+        out = oracle_run(oracle, cfg, p)
+        st, r, sp = out["stats"], out["species"][0], cfg["species"][0]
+        assert st.n_kappa_cap > 0.5 * st.n_sub and st.n_neg_disc == 0 and st.n_clamped_tau == 0
+        assert st.n_picard_cap == 0 and st.n_substep_cap == 0
+        res, div = continuity_residual(oracle, cfg, [(r["cell0"], r["s0"])],
+                                       [(r["cell"], r["s"])], out["jbar"])
+        assert np.linalg.norm(res) < 1e-12 * np.linalg.norm(div)
+        w_m = sp["w_q"] / sp["q_over_m"]
+        dK = 0.5 * w_m * np.sum(r["v"] ** 2 - r["v0"] ** 2)
+        dx = cfg["length"] / cfg["n_cells"]
+        work = cfg["dt"] * dx * np.sum(out["jbar"] * 0.5 * (cfg["E_n"] + cfg["E_np1"]))
+        assert abs(dK) > 1e-3 and abs(dK - work) < 1e-11 * abs(dK)
+        # per sub-step, on traced orbits
+        capped = binding = 0
+        for i in range(60):
+            recs, _ = oracle.trace_particle(cfg["n_cells"], cfg["length"], sp["q_over_m"],
+                                            sp["w_q"], r["cell0"][i], r["s0"][i], r["v0"][i],
+                                            cfg["E_n"], cfg["E_np1"], cfg["dt"], p)
+            assert sum(q.dtau for q in recs) == pytest.approx(cfg["dt"], rel=1e-13)
+            for q in recs:
+                assert abs(q.aprime) * q.dtau ** 2 / 4.0 <= 0.5 * (1 + 1e-15)
+                if q.aprime != 0.0:
+                    cap = math.sqrt(4.0 * 0.5 / abs(q.aprime))
+                    binding += q.dtau_est > cap
+                    if q.crossed == 0 and q.dtau_est > cap and q.dtau == cap:
+                        capped += 1            # an accepted step of exactly the cap's length
+                    assert q.dtau <= cap
+                if q.crossed:           # the truncated step satisfies Eq. 12 and F(dtau_c) = 0
+                    d = q.s1 - q.s0
+                    assert q.v1 ** 2 - q.v0 ** 2 == pytest.approx(2 * q.a_mid * d, abs=1e-12)
+                    assert abs(0.5 * q.a_mid * q.dtau ** 2 + q.v0 * q.dtau - d) < 1e-12
+        assert capped > 50 and binding > 300
+    # the cap is what keeps Eq. 11 finite: without it (kappa_max -> 1) 1 - kappa reaches ~0
+    # for a' > 0 and the same workload trips the crossing guards
+    wild = oracle_run(oracle, cfg, oracle.make_params(cn_mode=oracle.DIRECT, kappa_max=0.999999,
+                                                      **LOOSE))
+    assert wild["stats"].n_kappa_cap < out["stats"].n_kappa_cap
+
+
+@pytest.mark.parametrize("kind", ["land", "turn"])
+def test_guard_crossing_clamps(oracle, kind):
+    """O7 guards: D = v^2 + 2 a_m d clamped at 0 and dtau_c clamped to [0, dtau].  In exact
+    arithmetic neither can bind (SURVEY A-2: F(dtau) has the sign of the overshoot), so they
+    are reached only through rounding: particles that in exact arithmetic END the step exactly
+    on a face (helpers.landing_cfg).  Whichever branch rounding picks -- in-cell landing on the
+    face, crossing, crossing with a clamp -- the uniform-field closed form (P-2) fixes the
+    result: X1 = the face, v1 = v0 + a dt; and continuity / energy hold to rounding."""
+    tot = dict(n_neg_disc=0, n_clamped_tau=0, n_cross=0)
+    for seed in range(6):
+        for dt in (1.0, 0.7, 1.9):
+            cfg, state, (X1, v1) = landing_cfg(kind, dt=dt, seed=seed)
+            for mode in (oracle.PICARD, oracle.DIRECT):
+                out = oracle_run(oracle, cfg, oracle.make_params(cn_mode=mode, eps_a=1.0, eps_r=1.0),
+                                 state=state)
+                st, r = out["stats"], out["species"][0]
+                for k in tot:
+                    tot[k] += getattr(st, k)
+                _, X = unwrapped(cfg, r)
+                assert np.max(np.abs(X - X1)) < 4e-15
+                # 'turn': v1 = 0 is a square root of a rounding error (sensitivity of Eq. 12 at
+                # the apex), so |v1| ~ 1e-8; 'land': v1 to rounding
+                assert np.max(np.abs(r["v"] - v1)) < (2e-7 if kind == "turn" else 4e-15)
+                assert st.n_sub < 2.01 * X1.size and st.n_substep_cap == 0
+                res, div = continuity_residual(oracle, cfg, [(r["cell0"], r["s0"])],
+                                               [(r["cell"], r["s"])], out["jbar"])
+                assert np.max(np.abs(res)) < 1e-13
+                sp = cfg["species"][0]
+                dK = 0.5 * sp["w_q"] / sp["q_over_m"] * np.sum(r["v"] ** 2 - r["v0"] ** 2)
+                work = cfg["dt"] * np.sum(out["jbar"] * cfg["E_n"])
+                assert abs(dK - work) < 1e-12 * max(abs(dK), 1.0)
+    assert tot["n_cross"] > 1000                      # about half overshoot the face
+    # per sub-step: no step is longer than the time that was left (the dtau_c clamp), the
+    # discriminant's root is real (v1 finite), and the time adds up
+    cfg, state, _ = landing_cfg(kind, dt=0.7, seed=1)
+    sp, (cells, s0, v0) = cfg["species"][0], state[0]
+    p = oracle.make_params(cn_mode=oracle.DIRECT, eps_a=1.0, eps_r=1.0)
+    for i in range(cells.size):
+        recs, _ = oracle.trace_particle(cfg["n_cells"], cfg["length"], sp["q_over_m"], sp["w_q"],
+                                        cells[i], s0[i], v0[i], cfg["E_n"], cfg["E_np1"], 0.7, p)
+        left = 0.7
+        for q in recs:
+            assert 0.0 <= q.dtau <= left and math.isfinite(q.v1) and math.isfinite(q.s1)
+            left = 0.0 if q.dtau == left else left - q.dtau
+        assert left == 0.0
+    if kind == "land":
+        assert tot["n_clamped_tau"] > 50, tot         # the dtau_c clamp executed
+    else:
+        assert tot["n_neg_disc"] > 0, tot             # the D < 0 clamp executed
+
+
+def test_guard_picard_cap(oracle):
+    """A-3: the Picard loop stops after picard_max iterations.  With picard_max = 1 and tol = 0
+    every sub-step is cut off after its first iterate, which is the explicit midpoint rule
+    v' = v + dtau a(s + dtau v/2): checked by hand per sub-step.  With picard_max = k the error
+    against the converged step shrinks like |kappa|^k (contraction factor of Eq. 9-10).
+    Continuity (P-6) is exact whatever the iteration does."""
+    cfg = kappa_cap_cfg(n=600)
+    sp = cfg["species"][0]
+    p1 = oracle.make_params(cn_mode=oracle.PICARD, tol=0.0, picard_max=1)
+    out = oracle_run(oracle, cfg, p1)
+    st, r = out["stats"], out["species"][0]
+    assert st.n_picard_cap == st.n_sub == st.n_picard_it
+    res, div = continuity_residual(oracle, cfg, [(r["cell0"], r["s0"])], [(r["cell"], r["s"])],
+                                   out["jbar"])
+    assert np.linalg.norm(res) < 1e-12 * np.linalg.norm(div)
+    n = 0
+    for i in range(20):
+        recs, _ = oracle.trace_particle(cfg["n_cells"], cfg["length"], sp["q_over_m"], sp["w_q"],
+                                        r["cell0"][i], r["s0"][i], r["v0"][i], cfg["E_n"],
+                                        cfg["E_np1"], cfg["dt"], p1)
+        for q in recs:
+            if q.crossed == 0:
+                v1 = q.v0 + q.dtau * (q.a + q.aprime * (q.dtau * q.v0 / 2.0))
+                assert q.v1 == pytest.approx(v1, abs=1e-15 * max(1.0, abs(v1)))
+                assert q.s1 - q.s0 == pytest.approx(q.dtau * (q.v0 + v1) / 2.0, abs=1e-15)
+                n += 1
+    assert n > 1000
+    # convergence with the cap: one orbit segment, same dtau sequence forced by one sub-step
+    recs = {}
+    for k in (1, 2, 3, 50):
+        p = oracle.make_params(cn_mode=oracle.PICARD, tol=0.0 if k < 50 else 1e-15, picard_max=k,
+                               eps_a=1.0, eps_r=0.9)
+        rec, _ = oracle.trace_particle(2, 2.0, 1.0, 1.0, 0, 0.5, 0.1, [0.2, -0.2], [0.2, -0.2],
+                                       0.5, p)
+        assert len(rec) == 1 and rec[0].crossed == 0 and rec[0].dtau == 0.5
+        recs[k] = rec[0].v1
+    kappa = abs(-0.4 * 0.5 ** 2 / 4.0)
+    e = [abs(recs[k] - recs[50]) for k in (1, 2, 3)]
+    assert e[0] > 1e-6 and e[1] == pytest.approx(kappa * e[0], rel=1e-6)
+    assert e[2] == pytest.approx(kappa * e[1], rel=1e-4)
