@@ -55,6 +55,9 @@ enum {
   PIC_FLAG_ONE_PER_LANE = 64, /* fp32 only: run the one-particle-per-lane kernel also where the
                               default two-particles-per-lane packed-FP32 kernel (FFMA2) applies;
                               both give bit-identical orbits (A/B timing, tests)               */
+  PIC_FLAG_EXACT_TIME = 128, /* fp32 only: exact accounting of the time used by the sub-steps
+                              (fp64 checkpoints of the remaining time, D:5) instead of a plain
+                              fp32 `r -= dtau`, whose rounding random-walks to ~ulp(dt) sqrt(n_sub) */
   PIC_FLAG_DEPOSIT_PER_VISIT = 16 /* deposit per cell visit with shared fp64 atomics
                               instead of the default end-point form (D:5); same jbar to rounding */
 };
@@ -68,7 +71,7 @@ typedef struct pic_grid {
 typedef struct pic_species {
   double q_over_m;         /* q/m of the species (a = (q/m) E, Eq. 5)                    */
   double macro_charge;     /* w_q: charge of one macro-particle (sum_p w_q / L = q n0)         */
-  int64_t n;               /* number of particles                                              */
+  int64_t n;               /* number of particles, 0 <= n <= 2^31 - 1 (int32 binning cursors)  */
 } pic_species;
 
 typedef struct pic_params {
@@ -129,7 +132,9 @@ int pic_set_step(pic_handle* h, const double* E_n, double dt, double tol);
 
 /* pic_residual — Ampere residual (north_star; S8(a) a9):
  *   R_f = eps0 (E^{n+1}_f - E^n_f)/dt + jbar_f - <jbar>,  <jbar> = mean over faces, eps0 = 1,
- * with jbar from pic_move_accumulate(E^n, E_np1, dt, tol).  resid_out[n_cells]. */
+ * with jbar from pic_move_accumulate(E^n, E_np1, dt, tol).  resid_out[n_cells].
+ * Returns PIC_ERR_SUBSTEP_CAP (the residual is still written) if any particle was cut off at
+ * max_substeps; checked when resid_out is a HOST pointer, as for pic_move_accumulate. */
 int pic_residual(pic_handle* h, const double* E_np1, double* resid_out);
 
 /* pic_commit — accept state n+1 of the last pic_move_accumulate as the new state n and re-bin

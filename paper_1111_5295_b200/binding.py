@@ -22,6 +22,7 @@ PIC_FLAG_COUNTS, PIC_FLAG_DIAG, PIC_FLAG_NO_STORE, PIC_FLAG_VSORT = 1, 2, 4, 8
 PIC_FLAG_DEPOSIT_PER_VISIT = 16
 PIC_FLAG_NO_DEPOSIT = 32
 PIC_FLAG_ONE_PER_LANE = 64
+PIC_FLAG_EXACT_TIME = 128
 PIC_ERR_SUBSTEP_CAP = -4
 
 EXPORTS = ["pic_init", "pic_move_accumulate", "pic_set_step", "pic_residual", "pic_commit",

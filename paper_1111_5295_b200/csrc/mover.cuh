@@ -65,6 +65,7 @@ struct MoverArgs {
   T c_rel;                     // 2 eps_r:              dtau_rel = c_rel (|A|+|u|) / (|A|+|dA u|)
   T c_cap;                     // sqrt(4 kappa_max):    dtau_cap = c_cap / sqrt(|dA|)
   T dt, tol;
+  double dt_exact;             // dt in fp64 (EXACT_T: the checkpointed remaining time starts here)
   double scale;                // w_q / dt : cell-unit deposit -> jbar contribution
   double* partial;             // [gridDim.x][n_cells] per-block sums (scaled)
   unsigned long long* queue;   // global index-range counter (zeroed before launch)
@@ -186,7 +187,25 @@ struct Lane {
   uint32_t idx;        // particle index
   int32_t have;        // 0 = lane empty, 1 = a particle (in flight or parked), 2 = parked
                        // because it was cut off at max_substeps (A-9)
+  T el;                // EXACT_T: time used since the last checkpoint (small, so its sums are
+  double rem;          //          accurate); remaining time at the last checkpoint, exact
 };
+
+// EXACT_T (fp32 only): `r -= dtau` rounds to ulp(r)/2 at every sub-step, a random
+// walk of ulp(dt) sqrt(n_sub)/2 in the integrated time (5e-5 at dt = 50 and 590 sub-steps: the
+// particle is then moved for dt - 5e-5 and v is off by a * 5e-5).  With EXACT_T the time used is
+// also summed in `el`, which stays below kGroup sub-steps and is therefore accurate to a few
+// 1e-8, and every kGroup rounds the checkpoint `rem` (fp64) takes it over exactly and r is set
+// to the correctly rounded remaining time again: r drifts for at most kGroup sub-steps and never
+// accumulates.  r keeps its role (step limit, exact 0 at the orbit end).
+template <typename T>
+__device__ __forceinline__ void time_checkpoint(T& r, T& el, double& rem) {
+  rem -= (double)el;
+  el = T(0);
+  // a parked lane (r = 0) stays parked whatever rounding left in rem; a negative remainder
+  // (the orbit ran a few 1e-9 long) parks it
+  r = (r > T(0)) ? tmax((T)rem, T(0)) : T(0);
+}
 
 // ENDPOINT: start-cell terms are collected in registers while consecutive particles of the lane
 // start in the same cell (they do: the state is binned by cell) and flushed when it changes.
@@ -348,7 +367,7 @@ __device__ __forceinline__ void block_flush(const MoverArgs<T>& a, const double*
 // the current cell, accept it if it stays in the cell, otherwise truncate it at the face.
 // CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.  The max_substeps cap (A-9) is checked by the
 // caller once every kInner sub-steps.
-template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2>
+template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2, bool EXACT_T>
 __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restrict__ sA,
                                         double* __restrict__ sF, Lane<T>& p,
                                         unsigned& picard_its, unsigned* diag) {
@@ -358,11 +377,12 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
   //   d = (|A| + |dA u|)^(-1/2)  (one rsqrt).
   // A-1 (alpha = 0): d = +inf, the first term is +inf and the second +inf or NaN; the IEEE
   // max/min drop the NaN, so dtau = min(cap, r) -- the same limit as flooring alpha.
+  const bool live = p.r > T(0);   // counters below count orbits in flight, not parked lanes
   const T A = fma(p.dA, p.xi, p.AL);
   const T absA = tabs(A);
   const T d = Prim<T>::rsqrt_est(absA + tabs(p.dA * p.u));
   T dtau = tmax((a.c_rel * (absA + tabs(p.u))) * d, a.c_abs) * d;
-  if (DIAG && dtau > p.cap) diag[ST_KAPPA_CAP]++;
+  if (DIAG && live && dtau > p.cap) diag[ST_KAPPA_CAP]++;
   dtau = tmin(tmin(dtau, p.cap), p.r);
 
   // ---- a3 / O5: Crank-Nicolson step over dtau with the linear field of the current cell (A-4).
@@ -386,21 +406,22 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
       const bool done = tabs(un - uk) <= a.tol * (tabs(un) + tabs(Am) * dtau);
       uk = un;
       if (done) break;
-      if (it >= a.picard_max) { if (DIAG) diag[ST_PICARD_CAP]++; break; }
+      if (it >= a.picard_max) { if (DIAG && live) diag[ST_PICARD_CAP]++; break; }
     }
-    picard_its += it;
+    if (live) picard_its += it;
     u1 = uk;
   }
   const T xi1 = fma(h, p.u + u1, p.xi);               // Eq. 9
   // exact per-particle sub-step count only in the counting build (DIAG); a parked lane (r = 0)
   // takes a zero-length step that changes nothing and is not counted
-  if (DIAG) { if (p.r > T(0)) p.ns++; }
+  if (DIAG) { if (live) p.ns++; }
 
   if (in_unit<T>(xi1)) {
     // ---- O6: accept (inclusive, A-5).
     p.xi = xi1;
     p.u = u1;
     p.r -= dtau;
+    if (EXACT_T) p.el += dtau;
   } else {
     // ---- a4 / O7: crossing.  Land on the face the tentative step left through.
     const bool right = xi1 > T(1);
@@ -446,6 +467,7 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     if (PER_VISIT) p.xa = p.xi;
     p.u = uc;
     p.r -= dtc;
+    if (EXACT_T) p.el += dtc;
     load_cell<T>(sA, a.c_cap, p, cw);
   }
 }
@@ -464,7 +486,7 @@ template <> struct LaunchCfg<float> {
   static constexpr int block = kBlock;
 };
 
-template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2>
+template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2, bool EXACT_T = false>
 __global__ void __launch_bounds__(LaunchCfg<T>::block, LaunchCfg<T>::min_blocks)
 mover_kernel(const MoverArgs<T> a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -492,7 +514,8 @@ mover_kernel(const MoverArgs<T> a) {
   Lane<T> p;
   p.have = 0;
   p.idx = 0;
-  p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xa = T(0);
+  p.xi = p.u = p.r = p.AL = p.dA = p.cap = p.xa = p.el = T(0);
+  p.rem = 0.0;
   p.c = p.c0 = 0; p.ns = p.nc = p.nr = 0;
   StartAcc acc;
   acc.cell = -1; acc.f0 = acc.f1 = 0.0;
@@ -561,6 +584,7 @@ mover_kernel(const MoverArgs<T> a) {
             p.u = a.v0[cand] * a.inv_dx;
             p.c = a.cell0[cand];
             p.r = a.dt;
+            if (EXACT_T) { p.rem = a.dt_exact; p.el = T(0); }
             p.xa = p.xi;
             p.c0 = p.c;
             p.ns = 0; p.nc = 0; p.nr = 0;
@@ -584,7 +608,8 @@ mover_kernel(const MoverArgs<T> a) {
       if (!DIAG) { if (p.r > T(0)) p.ns += kGroup; }
 #pragma unroll
       for (int g = 0; g < kGroup; ++g)
-        substep<T, CN_DIRECT, DIAG, PER_VISIT, POW2>(a, sA, sF, p, picard_its, diag);
+        substep<T, CN_DIRECT, DIAG, PER_VISIT, POW2, EXACT_T>(a, sA, sF, p, picard_its, diag);
+      if (EXACT_T) time_checkpoint<T>(p.r, p.el, p.rem);
       if (!__any_sync(kFull, p.r > T(0))) break;
     }
   }

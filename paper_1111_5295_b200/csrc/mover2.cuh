@@ -46,9 +46,9 @@ __host__ __device__ inline size_t mover2_smem_bytes(int n_cells) {
 // a vector load would need moves on the common path).
 __device__ __forceinline__ void load_cell3(const float4* cc, float& AL, float& dA, float& cap) {
   const unsigned addr = (unsigned)__cvta_generic_to_shared(cc);
-  asm("ld.volatile.shared.f32 %0, [%1];" : "=f"(AL) : "r"(addr));
-  asm("ld.volatile.shared.f32 %0, [%1+4];" : "=f"(dA) : "r"(addr));
-  asm("ld.volatile.shared.f32 %0, [%1+8];" : "=f"(cap) : "r"(addr));
+  asm volatile("ld.volatile.shared.f32 %0, [%1];" : "=f"(AL) : "r"(addr) : "memory");
+  asm volatile("ld.volatile.shared.f32 %0, [%1+4];" : "=f"(dA) : "r"(addr) : "memory");
+  asm volatile("ld.volatile.shared.f32 %0, [%1+8];" : "=f"(cap) : "r"(addr) : "memory");
 }
 
 template <int S> __device__ __forceinline__ float get(const float2& v) { return S ? v.y : v.x; }

@@ -148,6 +148,7 @@ int rebin_species(pic_handle* h, SpeciesState& S) {
   const int src = 1 - h->cur, dst = h->cur;
   const VKey vk = key_of(S);
   const long long nk = (long long)ng * S.nx * S.nv;
+  if (nk > h->n_keys) return set_err(h, PIC_ERR_STATE, "rebin: sort key larger than the binning scratch");
   PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (nk + 1), h->stream));
   hist_kernel<T><<<grid_for(S.n), 256, 0, h->stream>>>(S.n, S.cell[src], (const T*)S.xi[src],
                                                        (const T*)S.v[src], h->d_hist, vk);
@@ -206,7 +207,7 @@ int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species,
       (params->cn_mode != PIC_CN_PICARD && params->cn_mode != PIC_CN_DIRECT))
     return PIC_ERR_ARG;
   for (int s = 0; s < n_species; ++s)
-    if (species[s].n < 0 || species[s].n > 0xffffffffLL || !x[s] || !v[s] ||
+    if (species[s].n < 0 || species[s].n > 0x7fffffffLL || !x[s] || !v[s] ||
         species[s].q_over_m == 0.0)
       return PIC_ERR_ARG;
   int ndev = 0;
@@ -367,7 +368,16 @@ int pic_residual(pic_handle* h, const double* E_np1, double* resid_out) {
                                             h->d_jbar, h->d_resid);
   h->launches++;
   PIC_CUDA(h, cudaGetLastError());
-  return from_device(h, h->d_resid, resid_out);
+  // A-9: orbits cut off at max_substeps leave dt unused; report it with the residual (the count
+  // rides on the synchronisation the host copy needs anyway)
+  unsigned long long capped = 0;
+  const bool host_out = !is_device_ptr(resid_out);
+  if (host_out)
+    PIC_CUDA(h, cudaMemcpyAsync(&capped, h->d_stats + ST_SUBSTEP_CAP, sizeof capped,
+                                cudaMemcpyDeviceToHost, h->stream));
+  if ((rc = from_device(h, h->d_resid, resid_out)) != PIC_OK) return rc;
+  if (capped) return set_err(h, PIC_ERR_SUBSTEP_CAP, "particles cut off at max_substeps");
+  return PIC_OK;
 }
 
 int pic_copy_state(pic_handle* dst, pic_handle* src) {
@@ -376,8 +386,14 @@ int pic_copy_state(pic_handle* dst, pic_handle* src) {
   if (dst->grid.n_cells != src->grid.n_cells || dst->grid.length != src->grid.length ||
       dst->sp.size() != src->sp.size())
     return set_err(dst, PIC_ERR_ARG, "pic_copy_state: grids or species differ");
-  for (size_t s = 0; s < src->sp.size(); ++s)
+  for (size_t s = 0; s < src->sp.size(); ++s) {
     if (dst->sp[s].n != src->sp[s].n) return set_err(dst, PIC_ERR_ARG, "pic_copy_state: particle counts differ");
+    // dst takes over src's sort key: its binning scratch (d_hist, d_scan) must hold that many keys
+    const SpeciesState& A = src->sp[s];
+    if ((long long)dst->grid.n_cells * A.nx * A.nv > dst->n_keys)
+      return set_err(dst, PIC_ERR_ARG, "pic_copy_state: dst was created without PIC_FLAG_VSORT (or "
+                                       "with fewer sort keys) than src's binning needs");
+  }
   // src's pending work must be complete before dst's stream reads its buffers
   PIC_CUDA(dst, cudaStreamSynchronize(src->stream));
   for (size_t s = 0; s < src->sp.size(); ++s) {

@@ -81,6 +81,7 @@ int jfnk_core(pic_handle* h, pic_handle* hj, double* E, double dt, double tol,
   std::vector<double> Rj0(n);   // residual of the Jacobian handle at the Newton iterate
   std::vector<double> Ek(E, E + n), R(n), Rp(n), w(n), Ep(n);
   if ((rc = J.resid(Ek, R)) != PIC_OK && rc != PIC_ERR_SUBSTEP_CAP) return rc;
+  bool capped = rc == PIC_ERR_SUBSTEP_CAP;   // of the LAST true residual (the state to commit)
   const double r0 = nrm2(R);
   double rn = r0;
   int newton = 0, gm_total = 0;
@@ -163,6 +164,7 @@ int jfnk_core(pic_handle* h, pic_handle* hj, double* E, double dt, double tol,
     // ---- Newton update and new residual (stores state n+1)
     for (int i = 0; i < n; ++i) Ek[i] += dE[i];
     if ((rc = J.resid(Ek, R)) != PIC_OK && rc != PIC_ERR_SUBSTEP_CAP) return rc;
+    capped = rc == PIC_ERR_SUBSTEP_CAP;
     rn = nrm2(R);
     ++newton;
     conv = rn <= o.rtol * r0 || rn <= o.atol;
@@ -179,6 +181,9 @@ int jfnk_core(pic_handle* h, pic_handle* hj, double* E, double dt, double tol,
   for (int i = 0; i < n; ++i) E[i] = Ek[i];
   if (!conv)
     return set_err(h, PIC_ERR_STATE, "pic_jfnk_step: Newton did not converge (state not committed)");
+  if (capped)   // A-9: some orbits of the converged state did not use up dt
+    return set_err(h, PIC_ERR_SUBSTEP_CAP,
+                   "pic_jfnk_step: particles cut off at max_substeps (state not committed)");
   if ((rc = pic_commit(h)) != PIC_OK) return rc;
   if (dc) return pic_copy_state(hj, h);   // the Jacobian handle follows the committed state
   return PIC_OK;

@@ -13,31 +13,43 @@ namespace {
 
 // Dispatch over the kernel's template switches (CN mode, diagnostics, deposit mode, power-of-two
 // grid).
-template <typename T, bool P2, typename F>
+template <typename T, bool P2, bool XT, typename F>
 auto with_kernel_p(bool direct, bool diag, bool per_visit, F&& f) {
   const int key = (direct ? 4 : 0) | (diag ? 2 : 0) | (per_visit ? 1 : 0);
   switch (key) {
-    case 0: return f(mover_kernel<T, false, false, false, P2>);
-    case 1: return f(mover_kernel<T, false, false, true, P2>);
-    case 2: return f(mover_kernel<T, false, true, false, P2>);
-    case 3: return f(mover_kernel<T, false, true, true, P2>);
-    case 4: return f(mover_kernel<T, true, false, false, P2>);
-    case 5: return f(mover_kernel<T, true, false, true, P2>);
-    case 6: return f(mover_kernel<T, true, true, false, P2>);
-    default: return f(mover_kernel<T, true, true, true, P2>);
+    case 0: return f(mover_kernel<T, false, false, false, P2, XT>);
+    case 1: return f(mover_kernel<T, false, false, true, P2, XT>);
+    case 2: return f(mover_kernel<T, false, true, false, P2, XT>);
+    case 3: return f(mover_kernel<T, false, true, true, P2, XT>);
+    case 4: return f(mover_kernel<T, true, false, false, P2, XT>);
+    case 5: return f(mover_kernel<T, true, false, true, P2, XT>);
+    case 6: return f(mover_kernel<T, true, true, false, P2, XT>);
+    default: return f(mover_kernel<T, true, true, true, P2, XT>);
   }
 }
+// exact: the EXACT_T instantiation (fp32 only; the fp64 kernel's r is exact enough as it is)
 template <typename T, typename F>
-auto with_kernel(bool direct, bool diag, bool per_visit, bool pow2, F&& f) {
-  return pow2 ? with_kernel_p<T, true>(direct, diag, per_visit, f)
-              : with_kernel_p<T, false>(direct, diag, per_visit, f);
+auto with_kernel(bool direct, bool diag, bool per_visit, bool pow2, bool exact, F&& f) {
+  if constexpr (sizeof(T) == 4) {
+    if (exact)
+      return pow2 ? with_kernel_p<T, true, true>(direct, diag, per_visit, f)
+                  : with_kernel_p<T, false, true>(direct, diag, per_visit, f);
+  }
+  return pow2 ? with_kernel_p<T, true, false>(direct, diag, per_visit, f)
+              : with_kernel_p<T, false, false>(direct, diag, per_visit, f);
+}
+
+// fp32 time accounting (mover.cuh, EXACT_T): on request.
+bool exact_time(const pic_params& P, double dt) {
+  (void)dt;
+  return (P.flags & PIC_FLAG_EXACT_TIME) != 0;
 }
 
 template <typename T>
 cudaError_t set_smem_all(size_t bytes) {
   cudaError_t e = cudaSuccess;
-  for (int key = 0; key < 16 && e == cudaSuccess; ++key)
-    e = with_kernel<T>(key & 4, key & 2, key & 1, key & 8, [&](auto k) {
+  for (int key = 0; key < 32 && e == cudaSuccess; ++key)
+    e = with_kernel<T>(key & 4, key & 2, key & 1, key & 8, key & 16, [&](auto k) {
       return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     });
   return e;
@@ -46,7 +58,7 @@ cudaError_t set_smem_all(size_t bytes) {
 template <typename T>
 int occupancy(size_t bytes) {
   int nb = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, true, false, false, true>, LaunchCfg<T>::block, bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mover_kernel<T, true, false, false, true, false>, LaunchCfg<T>::block, bytes);
   return nb;
 }
 
@@ -85,6 +97,7 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
   a.c_rel = (T)(2.0 * P.eps_r);
   a.c_cap = (T)std::sqrt(4.0 * P.kappa_max);
   a.dt = (T)dt;
+  a.dt_exact = dt;
   // a Picard tolerance below a few ulp of the kernel precision can never be met (A-3)
   const double tol_floor = 4.0 * (sizeof(T) == 4 ? 1.1920929e-7 : 2.220446049250313e-16);
   a.tol = (T)std::max(tol, tol_floor);
@@ -96,9 +109,10 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
   // the counting build: exact per-particle sub-step counts and anomaly counters
   const bool diag = (P.flags & (PIC_FLAG_DIAG | PIC_FLAG_COUNTS)) != 0;
   const bool per_visit = (P.flags & PIC_FLAG_DEPOSIT_PER_VISIT) != 0 && !(P.flags & PIC_FLAG_NO_DEPOSIT);
+  const bool exact = sizeof(T) == 4 && exact_time(P, dt);
   if constexpr (sizeof(T) == 4) {
     // production fp32 path: two particles per lane, packed FP32 (mover2.cuh)
-    if (direct && !diag && !per_visit && a.wrap_mask != 0 && S.grid_blocks2 > 0 &&
+    if (direct && !diag && !per_visit && !exact && a.wrap_mask != 0 && S.grid_blocks2 > 0 &&
         !(P.flags & PIC_FLAG_ONE_PER_LANE)) {
       a.refill_threshold = (S.nv > 1 || S.nx > 1) ? kRefill2Vsort : kRefill2;
       a.tile = S.tile2;
@@ -111,7 +125,7 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
   S.last_blocks = S.grid_blocks;
   h->last_kernel = "mover_kernel";
   dim3 g(S.grid_blocks), b(LaunchCfg<T>::block);
-  with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, [&](auto k) {
+  with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, exact, [&](auto k) {
     k<<<g, b, h->smem_bytes, h->stream>>>(a);
     return cudaSuccess;
   });

@@ -152,17 +152,3 @@ def config1(ppc=2000, seed=DEFAULT_SEED):
 def config4(ppc=4000, seed=DEFAULT_SEED):
     """configs[4]: IAW, 512 cells, 4000 particles/cell/species, dt=5."""
     return _iaw("cfg4", 512, ppc, 5.0, seed)
-
-
-def round_to_fp32_state(cfg):
-    """For fp32 parity runs both sides get fp32-representable inputs: returns,
-    per species, cell = floor(x/dx), xi = fp32(x/dx - cell) (in-cell offset in cell units) and
-    v = fp32(v).  Pure representation change; no method arithmetic."""
-    dx = cfg["length"] / cfg["n_cells"]
-    out = []
-    for sp in cfg["species"]:
-        u = sp["x"] / dx
-        cell = np.clip(np.floor(u), 0, cfg["n_cells"] - 1).astype(np.int32)
-        xi = np.clip(u - cell, 0.0, 1.0).astype(np.float32)
-        out.append(dict(cell=cell, xi=xi, v=sp["v"].astype(np.float32)))
-    return out

@@ -5,11 +5,17 @@ import numpy as np
 
 from paper_1111_5295_b200 import binding as B
 from paper_1111_5295_b200 import workloads as W
-from helpers import continuity_residual, oracle_run, periodic_dist, rel_l2
+from helpers import (continuity_residual, oracle_run, periodic_dist, rel_l2,
+                     round_to_fp32_state)
 
 # north_star tolerances
 TOL = {"fp64": dict(x=1e-10, v=1e-10, j=1e-10, cont=1e-10),
        "fp32": dict(x=1e-5, v=1e-5, j=1e-4, cont=1e-5)}
+# max-norm gates beside the L2 ones: per non-flipped particle, |d xi| in cell units
+# and |d v| / v_rms.  A single orbit's error is the L2 figure times a tail factor (errors are
+# rounding random walks amplified by the orbit's own sensitivity); 100 x the L2 bar still
+# catches one bad particle in 1e5, which the L2 norm alone would let through 300-fold.
+TOL_MAX = {"fp64": dict(xi=1e-8, v=1e-8), "fp32": dict(xi=1e-3, v=1e-3)}
 
 
 def gpu_run(cfg, precision, cn_mode="direct", flags=B.PIC_FLAG_COUNTS | B.PIC_FLAG_DIAG,
@@ -43,7 +49,7 @@ def oracle_state_for(cfg, precision, subset=None):
     dx = cfg["length"] / cfg["n_cells"]
     st = []
     if precision == "fp32":
-        for j, r in enumerate(W.round_to_fp32_state(cfg)):
+        for j, r in enumerate(round_to_fp32_state(cfg)):
             idx = slice(None) if subset is None else subset[j]
             st.append((r["cell"][idx], r["xi"][idx].astype(np.float64) * dx,
                        r["v"][idx].astype(np.float64)))
@@ -63,7 +69,8 @@ def sub_cfg(cfg, subset):
     return out
 
 
-def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=0, fast=False):
+def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=0, fast=False,
+           pic_kw=None):
     """Run both sides; return metrics (SURVEY 8(c) 'Parity metrics').  Particles whose
     (n_sub, n_cross, cell) differ are branch flips (A-12): excluded from x/v, counted, and
     jbar is then recomputed on both sides on the non-flipped subset.
@@ -73,11 +80,12 @@ def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=
     counts that identify flips still come from a counting-build run, whose orbits must be
     bit-identical to the fast build's (asserted here)."""
     dx = cfg["length"] / cfg["n_cells"]
+    pic_kw = pic_kw or {}
     flags = B.PIC_FLAG_COUNTS | B.PIC_FLAG_DIAG | extra_flags
-    g = gpu_run(cfg, precision, cn_mode, flags=flags)
+    g = gpu_run(cfg, precision, cn_mode, flags=flags, **pic_kw)
     if fast:
         flags = extra_flags
-        gf = gpu_run(cfg, precision, cn_mode, flags=flags)
+        gf = gpu_run(cfg, precision, cn_mode, flags=flags, **pic_kw)
         gf["kernel"] = gf["pic"].last_kernel()
         for a, b in zip(gf["species"], g["species"]):
             for k in ("x", "v", "cell", "xi"):
@@ -88,7 +96,8 @@ def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=
         g = gf
     oc = sub_cfg(cfg, [slice(None)] * len(cfg["species"]))
     ref = oracle_run(o, oc, oracle_params, state=oracle_state_for(cfg, precision))
-    m = dict(flips=0, n=0, x=[], v=[], stats=g["stats"], ostats=ref["stats"].as_dict())
+    m = dict(flips=0, n=0, x=[], v=[], xi_max=[], v_max=[], stats=g["stats"],
+             ostats=ref["stats"].as_dict())
     keep = []
     for gs, rs in zip(g["species"], ref["species"]):
         same = (gs["n_sub"] == rs["n_sub"]) & (gs["n_cross"] == rs["n_cross"]) & \
@@ -100,11 +109,17 @@ def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=
         d = periodic_dist(gs["x"][same], xr[same], cfg["length"])
         m["x"].append(float(np.linalg.norm(d) / max(np.linalg.norm(xr[same]), 1e-300)))
         m["v"].append(rel_l2(gs["v"][same], rs["v"][same]))
+        # max norms over the non-flipped particles: position error in CELL units, velocity error
+        # relative to the species' rms speed (one bad orbit cannot hide inside an L2 norm)
+        m["xi_max"].append(float(d.max() / dx) if d.size else 0.0)
+        vrms = float(np.sqrt(np.mean(rs["v"] ** 2))) if rs["v"].size else 1.0
+        m["v_max"].append(float(np.max(np.abs(gs["v"][same] - rs["v"][same])) / max(vrms, 1e-300))
+                          if d.size else 0.0)
     if m["flips"] == 0:
         gj, rj = g["jbar"], ref["jbar"]
     else:
         sub = [np.nonzero(k)[0] for k in keep]
-        g2 = gpu_run(cfg, precision, cn_mode, flags=flags, subset=sub)
+        g2 = gpu_run(cfg, precision, cn_mode, flags=flags, subset=sub, **pic_kw)
         r2 = oracle_run(o, sub_cfg(cfg, sub), oracle_params,
                         state=oracle_state_for(cfg, precision, sub))
         gj, rj = g2["jbar"], r2["jbar"]
@@ -120,8 +135,12 @@ def parity(o, cfg, precision, cn_mode="direct", oracle_params=None, extra_flags=
     return m
 
 
-def assert_parity(m, precision, max_flip_frac=1e-3):
+def assert_parity(m, precision, max_flip_frac=1e-3, max_norms=True):
     t = TOL[precision]
+    if max_norms:
+        tm = TOL_MAX[precision]
+        assert max(m["xi_max"]) <= tm["xi"], f"max |d xi| {max(m['xi_max'])} cells > {tm['xi']}"
+        assert max(m["v_max"]) <= tm["v"], f"max |d v|/v_rms {max(m['v_max'])} > {tm['v']}"
     assert m["flips"] <= max_flip_frac * m["n"], f"too many branch flips: {m['flips']}/{m['n']}"
     for x in m["x"]:
         assert x <= t["x"], f"x rel L2 {x} > {t['x']}"

@@ -56,6 +56,20 @@ def continuity_residual(o, cfg, start, end, jbar):
     return rho1 - rho0 + div, div
 
 
+def round_to_fp32_state(cfg):
+    """For fp32 parity runs both sides get fp32-representable inputs: returns,
+    per species, cell = floor(x/dx), xi = fp32(x/dx - cell) (in-cell offset in cell units) and
+    v = fp32(v).  Pure representation change; no method arithmetic."""
+    dx = cfg["length"] / cfg["n_cells"]
+    out = []
+    for sp in cfg["species"]:
+        u = sp["x"] / dx
+        cell = np.clip(np.floor(u), 0, cfg["n_cells"] - 1).astype(np.int32)
+        xi = np.clip(u - cell, 0.0, 1.0).astype(np.float32)
+        out.append(dict(cell=cell, xi=xi, v=sp["v"].astype(np.float32)))
+    return out
+
+
 # ---- workloads that EXECUTE the guard branches of the mover (SURVEY 8(c) A-2, A-3, O7) ----------
 # Input design only (kinematics of a uniformly accelerated particle); no arithmetic of the method.
 def kappa_cap_cfg(n=4000, seed=9):
@@ -109,3 +123,36 @@ def landing_cfg(kind, n_cells=4096, dt=1.0, seed=3, q_over_m=-1.0):
                species=[dict(name="e", q_over_m=q_over_m, w_q=-float(n_cells) / m, x=x, v=v0)])
     X1 = cells + np.where(sgn > 0, 1.0, 0.0)
     return cfg, [(cells, s0, v0)], (X1, v0 + a * dt)
+
+
+def ulp_response(o, cfg, seed=1):
+    """How much the METHOD amplifies one fp32 rounding error (cfg3): run the oracle
+    (fp64) twice from fp32-representable inputs that differ by one fp32 ulp in every particle's
+    velocity (random sign), and return the relative L2 response of x, v (over the particles that
+    took the same branches) and jbar, plus the mean sub-steps per particle.  An fp32 kernel makes
+    such an error at every one of its n_sub sub-steps, so its distance from the oracle is about
+    response x sqrt(n_sub) (random walk) whatever its arithmetic."""
+    dx = cfg["length"] / cfg["n_cells"]
+    rng = np.random.default_rng(seed)
+    st0, st1 = [], []
+    for r in round_to_fp32_state(cfg):
+        s = r["xi"].astype(np.float64) * dx
+        toward = np.where(rng.random(r["v"].size) < 0.5, -np.inf, np.inf).astype(np.float32)
+        v1 = np.nextafter(r["v"], toward)
+        st0.append((r["cell"], s, r["v"].astype(np.float64)))
+        st1.append((r["cell"], s, v1.astype(np.float64)))
+    p = o.make_params(cn_mode=o.DIRECT)
+    a, b = oracle_run(o, cfg, p, state=st0), oracle_run(o, cfg, p, state=st1)
+    out = dict(x=0.0, v=0.0, flips=0)
+    for ra, rb in zip(a["species"], b["species"]):
+        same = (ra["n_sub"] == rb["n_sub"]) & (ra["n_cross"] == rb["n_cross"]) & \
+               (ra["cell"] == rb["cell"])
+        out["flips"] += int((~same).sum())
+        xa = ra["cell"] * dx + ra["s"]
+        d = periodic_dist(xa[same], (rb["cell"] * dx + rb["s"])[same], cfg["length"])
+        out["x"] = max(out["x"], float(np.linalg.norm(d) / np.linalg.norm(xa[same])))
+        out["v"] = max(out["v"], rel_l2(rb["v"][same], ra["v"][same]))
+    out["j"] = rel_l2(b["jbar"], a["jbar"])
+    n = sum(r["n_sub"].size for r in a["species"])
+    out["n_sub_mean"] = a["stats"].n_sub / n
+    return out

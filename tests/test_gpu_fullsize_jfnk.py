@@ -136,10 +136,21 @@ def test_defect_correction_matches_fp64(oracle):
     E_ref = gauss_field(ref.rho(B.PIC_STATE_N), dx)
     E_dc = E_ref.copy()
     e0 = float(h64.kinetic_energy(B.PIC_STATE_N).sum() + 0.5 * dx * np.sum(E_dc * E_dc))
+    import gpu_helpers as G
     for step in range(3):
+        En = E_dc.copy()
+        before = [h64.get_particles(j, B.PIC_STATE_N) for j in range(2)]
         ia = ref.jfnk_step(E_ref, dt, rtol=1e-9)
         ib = h64.jfnk_step(E_dc, dt, rtol=1e-9, jacobian=h32)
         assert ia["converged"] == 1 and ib["converged"] == 1, (ia, ib)
+        # the ORACLE's residual at the field the defect-correction solve converged to, from the
+        # same state n: as small as the solver's own (DP accuracy with SP products)
+        state = [(b["cell"], b["xi"] * dx, b["v"]) for b in before]
+        oref = G.oracle_run(oracle, dict(cfg, E_n=En, E_np1=E_dc),
+                            oracle.make_params(cn_mode=oracle.DIRECT), state=state)
+        Ro = np.linalg.norm(oracle.residual(En, E_dc, dt, oref["jbar"]))
+        print(f"[dc] step {step}: oracle |R| at the dc solution = {Ro:.2e} (|R0| {ib['resid0']:.2e})")
+        assert Ro <= 1e-7 * ib["resid0"]
         err = np.linalg.norm(E_dc - E_ref) / np.linalg.norm(E_ref)
         print(f"[dc] step {step}: fp64 newton={ia['newton_its']} calls={ia['mover_calls']} | "
               f"dc newton={ib['newton_its']} calls={ib['mover_calls']} of which fp64 "
