@@ -228,7 +228,8 @@ const char* pic_last_kernel(const pic_handle* h);
  * of one instruction class in 1e9 thread-operations per second over the whole chip, from a
  * full-occupancy kernel of independent dependent chains timed with CUDA events (divide by n_sm
  * and the SM clock for operations per clock and SM).  which: 0 FFMA, 1 FFMA2 (packed; counts two
- * per thread), 2 FMNMX (ALU pipe), 3 MUFU.RSQ, 4 DFMA, 5 the mix 4 FFMA2 + 4 FMNMX per iteration.
+ * per thread), 2 FMNMX (ALU pipe), 3 MUFU.RSQ, 4 DFMA, 5 the mix 4 FFMA2 + 4 FMNMX per iteration,
+ * 6 the mix 8 FFMA + 4 FMNMX, 7 4 FFMA + 4 FMNMX, 8 2 FFMA2 + 4 FFMA + 4 FMNMX, 9 4 FFMA2 + 2 MUFU.
  * iters: loop length (e.g. 20000).  n_sm may be NULL.  Needs no handle; runs on the default
  * stream and synchronises it. */
 int pic_microbench(int which, int iters, double* thread_gops, int* n_sm);

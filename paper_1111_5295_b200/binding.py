@@ -125,7 +125,8 @@ def _check_f64(a, n, name):
         raise ValueError(f"{name}: need float64[{n}]")
 
 
-MICROBENCH = {0: "ffma", 1: "ffma2", 2: "fmnmx", 3: "mufu_rsq", 4: "dfma", 5: "ffma2+fmnmx"}
+MICROBENCH = {0: "ffma", 1: "ffma2", 2: "fmnmx", 3: "mufu_rsq", 4: "dfma", 5: "ffma2+fmnmx",
+              6: "8ffma+4fmnmx", 7: "4ffma+4fmnmx", 8: "2ffma2+4ffma+4fmnmx", 9: "4ffma2+2mufu"}
 
 
 def microbench(iters=20000, sm_mhz=1965.0):

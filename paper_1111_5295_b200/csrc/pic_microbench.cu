@@ -61,11 +61,40 @@ __global__ void __launch_bounds__(kThreads) ubench_kernel(int iters, float s, fl
     } else if (WHICH == 4) {
 #pragma unroll
       for (int i = 0; i < kChains; ++i) q[i] = dfma1(q[i], qb, qc);
-    } else {
+    } else if (WHICH == 5) {
 #pragma unroll
       for (int i = 0; i < kChains / 2; ++i) p[i] = ffma2(p[i], pb, pc);
 #pragma unroll
       for (int i = 0; i < kChains / 2; ++i) a[i] = (it & 1) ? fmax1(a[i], c) : -fmax1(-a[i], -b);
+    } else if (WHICH == 6) {
+      // 8 scalar FFMA + 4 FMNMX: the same FMA work as mix 5 in scalar form
+#pragma unroll
+      for (int i = 0; i < kChains / 2; ++i) {
+        p[i] = ((unsigned long long)__float_as_uint(ffma1(__uint_as_float((unsigned)(p[i] >> 32)), b, c)) << 32) |
+               __float_as_uint(ffma1(__uint_as_float((unsigned)p[i]), b, c));
+      }
+#pragma unroll
+      for (int i = 0; i < kChains / 2; ++i) a[i] = (it & 1) ? fmax1(a[i], c) : -fmax1(-a[i], -b);
+    } else if (WHICH == 7) {
+      // 4 scalar FFMA + 4 FMNMX
+#pragma unroll
+      for (int i = 0; i < kChains / 2; ++i) a[i + kChains / 2] = ffma1(a[i + kChains / 2], b, c);
+#pragma unroll
+      for (int i = 0; i < kChains / 2; ++i) a[i] = (it & 1) ? fmax1(a[i], c) : -fmax1(-a[i], -b);
+    } else if (WHICH == 8) {
+      // 2 FFMA2 + 4 scalar FFMA + 4 FMNMX
+      p[0] = ffma2(p[0], pb, pc);
+      p[1] = ffma2(p[1], pb, pc);
+#pragma unroll
+      for (int i = 0; i < kChains / 2; ++i) a[i + kChains / 2] = ffma1(a[i + kChains / 2], b, c);
+#pragma unroll
+      for (int i = 0; i < kChains / 2; ++i) a[i] = (it & 1) ? fmax1(a[i], c) : -fmax1(-a[i], -b);
+    } else {
+      // 4 FFMA2 + 2 MUFU.RSQ
+#pragma unroll
+      for (int i = 0; i < kChains / 2; ++i) p[i] = ffma2(p[i], pb, pc);
+      a[0] = rsq1(a[0]);
+      a[1] = rsq1(a[1]);
     }
   }
   float r = 0.0f;
@@ -89,7 +118,7 @@ cudaError_t run(int blocks, int iters, float* sink, cudaEvent_t e0, cudaEvent_t 
 }  // namespace
 
 extern "C" int pic_microbench(int which, int iters, double* thread_gops, int* n_sm) {
-  if (which < 0 || which > 5 || iters < 1 || !thread_gops) return PIC_ERR_ARG;
+  if (which < 0 || which > 9 || iters < 1 || !thread_gops) return PIC_ERR_ARG;
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) != cudaSuccess ||
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
@@ -109,7 +138,11 @@ extern "C" int pic_microbench(int which, int iters, double* thread_gops, int* n_
       case 2: e = run<2>(blocks, iters, sink, e0, e1); break;
       case 3: e = run<3>(blocks, iters, sink, e0, e1); break;
       case 4: e = run<4>(blocks, iters, sink, e0, e1); break;
-      default: e = run<5>(blocks, iters, sink, e0, e1); break;
+      case 5: e = run<5>(blocks, iters, sink, e0, e1); break;
+      case 6: e = run<6>(blocks, iters, sink, e0, e1); break;
+      case 7: e = run<7>(blocks, iters, sink, e0, e1); break;
+      case 8: e = run<8>(blocks, iters, sink, e0, e1); break;
+      default: e = run<9>(blocks, iters, sink, e0, e1); break;
     }
   }
   float ms = 0.0f;
@@ -120,7 +153,10 @@ extern "C" int pic_microbench(int which, int iters, double* thread_gops, int* n_
   if (e != cudaSuccess || !(ms > 0.0f)) { cudaGetLastError(); return PIC_ERR_CUDA; }
   // thread-operations of the launch: blocks x kThreads x iters x kChains (FFMA2 counts as two
   // thread-operations; the mix has kChains/2 FFMA2 + kChains/2 FMNMX per iteration)
-  const double per_iter = which == 1 ? 2.0 * kChains : which == 5 ? 1.5 * kChains : kChains;
+  // mixes 6-9: thread-operations per iteration = 8+4, 4+4, 4+4+4, 8+2 (FFMA2 counts two)
+  const double per_iter = which == 1 ? 2.0 * kChains : which == 5 ? 1.5 * kChains
+                        : which == 6 ? 12.0 : which == 7 ? 8.0 : which == 8 ? 12.0
+                        : which == 9 ? 10.0 : kChains;
   *thread_gops = (double)blocks * kThreads * (double)iters * per_iter / ((double)ms * 1e6);
   if (n_sm) *n_sm = sms;
   return PIC_OK;

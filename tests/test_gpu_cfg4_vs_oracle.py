@@ -1,0 +1,118 @@
+"""`-m gpu`: BASELINE.json configs[4] as it states it -- the long ion-acoustic-wave run with the
+fp32 GPU mover under the host fp64 JFNK, "reported against the fp64 ORACLE run for the first 20
+steps" (the paper's Fig. 6 compares the hybrid run with the CPU-only double-precision run,
+PAPER.md:321-323).  Full size: 512 cells, 2 x 2,048,000 particles, dt = 5.
+
+Three runs from the same initial state: the oracle under tests/oracle_jfnk.py (rtol 1e-8), the
+fp64 GPU mover under pic_jfnk_step (rtol 1e-8), the fp32 GPU mover (rtol 2e-4, SURVEY A-14).
+Per step: field / electron / ion energies, total-energy change, Gauss-law residual (local charge
+conservation), Newton and GMRES counts, wall time.  The table goes to
+gpurun_out/cfg4_vs_oracle.json (summarised in profiles/)."""
+import json
+import os
+import time
+
+import numpy as np
+import pytest
+
+from paper_1111_5295_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+STEPS = int(os.environ.get("PIC_CFG4_STEPS", "20"))
+
+
+def _gauss(E, rho, dx):
+    return float(np.linalg.norm((np.roll(E, -1) - E) / dx - rho) / max(np.linalg.norm(rho), 1e-300))
+
+
+def test_cfg4_first_steps_against_the_oracle(oracle):
+    from oracle_jfnk import OracleIAW
+    from paper_1111_5295_b200 import binding as B
+    from paper_1111_5295_b200.iaw import gauss_field
+    cfg = W.config4()
+    ng, L, dt = cfg["n_cells"], cfg["length"], cfg["dt"]
+    dx = L / ng
+    runs = {}
+
+    # ---- the oracle under the harness-side Newton-Krylov
+    S = OracleIAW(oracle, cfg, oracle.make_params(cn_mode=oracle.DIRECT))
+    E = S.gauss_field()
+    E0 = E.copy()
+    hist = []
+    for n in range(STEPS):
+        t0 = time.perf_counter()
+        E, info = S.step(E, rtol=1e-8)
+        wall = time.perf_counter() - t0
+        assert info["converged"] == 1, info
+        ke = S.kinetic()
+        hist.append(dict(step=n + 1, ke=ke, field=float(0.5 * dx * np.sum(E * E)),
+                         gauss=_gauss(E, S.rho(), dx), newton=info["newton_its"],
+                         gmres=info["gmres_its"], mover_calls=info["mover_calls"], wall_s=wall,
+                         E=E.copy()))
+    runs["oracle fp64 (rtol 1e-8, %d host cores)" % S.cores] = hist
+    S.close()
+
+    # ---- the GPU movers under pic_jfnk_step
+    for name, precision, rtol in (("gpu fp64 (rtol 1e-8)", "fp64", 1e-8),
+                                  ("gpu fp32 (rtol 2e-4)", "fp32", 2e-4)):
+        pic = B.Pic(ng, L, cfg["species"], precision=precision, cn_mode="direct", flags=B.PIC_FLAG_VSORT)
+        E = gauss_field(pic.rho(B.PIC_STATE_N), dx)
+        # same start (A-13); both species carry the same density perturbation, so rho = 0 and
+        # E^0 is zero to rounding: compare absolutely
+        assert np.max(np.abs(E - E0)) <= 1e-12
+        hist = []
+        for n in range(STEPS):
+            t0 = time.perf_counter()
+            info = pic.jfnk_step(E, dt, rtol=rtol)
+            wall = time.perf_counter() - t0
+            assert info["converged"] == 1, info
+            hist.append(dict(step=n + 1, ke=[float(k) for k in pic.kinetic_energy(B.PIC_STATE_N)],
+                             field=float(0.5 * dx * np.sum(E * E)),
+                             gauss=_gauss(E, pic.rho(B.PIC_STATE_N), dx), newton=info["newton_its"],
+                             gmres=info["gmres_its"], mover_calls=info["mover_calls"], wall_s=wall,
+                             E=E.copy()))
+        runs[name] = hist
+        pic.close()
+
+    names = list(runs)
+    ref = runs[names[0]]
+    table = {}
+    for name in names:
+        h = runs[name]
+        tot = np.array([sum(r["ke"]) + r["field"] for r in h])
+        drift = np.abs(np.diff(tot)) / tot[0]
+        dE = [float(np.linalg.norm(r["E"] - q["E"]) / np.linalg.norm(q["E"])) for r, q in zip(h, ref)]
+        table[name] = dict(
+            newton_mean=float(np.mean([r["newton"] for r in h])),
+            gmres_mean=float(np.mean([r["gmres"] for r in h])),
+            mover_calls_mean=float(np.mean([r["mover_calls"] for r in h])),
+            wall_ms_per_step=float(1e3 * np.mean([r["wall_s"] for r in h])),
+            max_energy_change_per_step=float(drift.max()) if drift.size else 0.0,
+            energy_change_over_run=float(abs(tot[-1] - tot[0]) / tot[0]),
+            max_gauss=float(max(r["gauss"] for r in h)),
+            field_rel_diff_vs_oracle=dict(step1=dE[0], mid=dE[len(dE) // 2], last=dE[-1]),
+            ke_e_rel_diff_vs_oracle_last=float(abs(h[-1]["ke"][0] - ref[-1]["ke"][0]) / ref[-1]["ke"][0]),
+            ke_i_rel_diff_vs_oracle_last=float(abs(h[-1]["ke"][1] - ref[-1]["ke"][1]) / ref[-1]["ke"][1]),
+            field_energy_rel_diff_vs_oracle_last=float(abs(h[-1]["field"] - ref[-1]["field"]) / ref[-1]["field"]),
+            history=[dict((k, v) for k, v in r.items() if k != "E") for r in h])
+        print(f"[cfg4] {name}: " + json.dumps({k: v for k, v in table[name].items() if k != "history"}))
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(os.path.join("gpurun_out", "cfg4_vs_oracle.json"), "w") as f:
+        json.dump(dict(config="BASELINE.json configs[4]", n_cells=ng, particles=[int(sp["x"].shape[0]) for sp in cfg["species"]],
+                       dt=dt, steps=STEPS, runs=table), f, indent=1)
+
+    o, g64, g32 = (table[n] for n in names)
+    # the fp64 GPU run IS the oracle run to the nonlinear tolerance, step after step
+    assert g64["field_rel_diff_vs_oracle"]["last"] < 1e-6
+    assert g64["ke_e_rel_diff_vs_oracle_last"] < 1e-9 and g64["ke_i_rel_diff_vs_oracle_last"] < 1e-9
+    # energy: conserved to the nonlinear tolerance level: 1e-8-class for fp64, the fp32
+    # hybrid at its looser tolerance
+    assert o["max_energy_change_per_step"] < 1e-9 and g64["max_energy_change_per_step"] < 1e-9
+    assert g32["max_energy_change_per_step"] < 5e-6
+    # local charge conservation (Gauss's law stays satisfied): exact for both precisions, since
+    # the deposit is an exact function of the stored end points
+    assert o["max_gauss"] < 1e-6 and g64["max_gauss"] < 1e-6
+    # the fp32 hybrid tracks the oracle's macroscopic quantities to its tolerance
+    assert g32["ke_e_rel_diff_vs_oracle_last"] < 1e-4
+    assert g32["field_energy_rel_diff_vs_oracle_last"] < 5e-3
