@@ -37,6 +37,12 @@ OPS_INCELL, OPS_CROSS = 43.0, 72.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one mover launch from the committed
 # `ncu --set full` capture (profiles/r1_mover_ncu.md); known only for the default workload.
 NCU_TRAFFIC_BYTES = {("cfg2", 100_000_000, "fp32"): 2.366e9}
+NCU_TRAFFIC_SOURCE = "profiles/r2_mover_ncu.md (ncu --set full capture of this kernel; not measured in this run)"
+# Executed thread-operations per sub-step of the timed kernel, summed over the SASS lines of the
+# same ncu capture (source page, predicated-on thread instructions): (a) the paper's convention
+# (every instruction 1, FFMA 2, packed FFMA2 4, FMUL2 / FADD2 2), (b) floating-point arithmetic
+# only (FADD, FMUL, FFMA, their packed forms; no integer, compare, select, MUFU, memory, control).
+NCU_EXECUTED_OPS = {("cfg2", 100_000_000, "fp32", "mover2_kernel"): (45.45, 27.48)}
 
 
 def _workload(name, n, seed):
@@ -46,6 +52,10 @@ def _workload(name, n, seed):
         return W.config3(n=n or 20_000_000, seed=seed)
     if name == "cfg0":
         return W.config0(n=n or 6400, seed=seed)
+    if name == "cfg1":
+        return W.config1(ppc=(n // 512) if n else 2000, seed=seed)
+    if name == "cfg4":
+        return W.config4(ppc=(n // 1024) if n else 4000, seed=seed)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -143,6 +153,8 @@ def run_reference(args, rank, world):
     """--impl reference: the oracle on the host cores, bounded sample per step."""
     if rank != 0:
         return
+    if args.workload in ("cfg1", "cfg4"):
+        return run_reference_iaw(args, world)
     sample = args.ref_sample
     cfg = _workload(args.workload, sample, args.seed)
     for _ in range(args.warmup):
@@ -166,24 +178,208 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def run_reference_iaw(args, world):
+    """--impl reference on configs[1] / [4]: the implicit step driven by the oracle (the
+    harness-side Newton-Krylov of tests/oracle_jfnk.py around oracle.move_accumulate), all host
+    cores, on a bounded sample: the same grid and dt with 1/20 of the particles per cell."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from oracle import pic_oracle as o
+    from oracle_jfnk import OracleIAW
+    o.build()
+    full = 2000 if args.workload == "cfg1" else 4000
+    ppc = max(full // 20, 10)
+    cfg = (W.config1 if args.workload == "cfg1" else W.config4)(ppc=ppc, seed=args.seed)
+    S = OracleIAW(o, cfg, o.make_params(cn_mode=o.DIRECT))
+    E = S.gauss_field()
+    for _ in range(args.warmup):
+        E, _ = S.step(E, rtol=1e-8)
+    tot_sub, t0 = 0, time.perf_counter()
+    for _ in range(args.steps):
+        c0 = S.mover_calls
+        E, info = S.step(E, rtol=1e-8)
+        tot_sub += S.last_n_sub * (S.mover_calls - c0)
+    tot_t = time.perf_counter() - t0
+    val = tot_sub / tot_t
+    desc = (f"{args.workload} grid and dt with {ppc} of {full} particles per cell per species, "
+            f"implicit steps (rtol 1e-8) driven by the fp64 oracle on {S.cores} host cores")
+    S.close()
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                      "data": "synthetic", "config": {"workload": args.workload, "sample": desc},
+                      "cpu_baseline": {"value": val, "unit": UNIT, "cores": S.cores, "kind": "oracle", "sample": desc},
+                      "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                      "gpu_launches": 0}), flush=True)
+
+
+def run_iaw(args, rank, world, local_rank, explicit_steps):
+    """configs[1] / configs[4]: a "step" is one fully implicit time step (pic_jfnk_step: host fp64
+    Newton-GMRES, one GPU mover pass per residual, commit + re-binning on convergence; P:111,
+    P:321).  value = particle sub-steps of all mover passes of the timed steps / their time; the
+    host E in / residual out copies of every pass are inside it (that IS the method's boundary,
+    P:31), so e2e = value."""
+    import torch
+    import torch.distributed as dist
+    from paper_1111_5295_b200 import binding as B
+    from paper_1111_5295_b200 import replicas
+    from paper_1111_5295_b200.iaw import gauss_field
+    cfg = _workload(args.workload, args.n, replicas.rank_seed(args.seed, rank))
+    ng, L, dt = cfg["n_cells"], cfg["length"], cfg["dt"]
+    dx = L / ng
+    rtol = args.rtol or (1e-8 if args.precision == "fp64" else 2e-4)     # SURVEY A-14
+    stream = torch.cuda.current_stream().cuda_stream
+    flags = 0 if args.no_vsort else B.PIC_FLAG_VSORT
+    pic = B.Pic(ng, L, cfg["species"], precision=args.precision, cn_mode=args.cn_mode, flags=flags,
+                stream=stream)
+    jac = None
+    if args.defect_correction:
+        jac = B.Pic(ng, L, cfg["species"], precision="fp32", cn_mode=args.cn_mode, flags=flags, stream=stream)
+    n_p = sum(pic.n)
+    E = gauss_field(pic.rho(B.PIC_STATE_N), dx)
+
+    def energy():
+        return float(pic.kinetic_energy(B.PIC_STATE_N).sum() + 0.5 * dx * np.sum(E * E))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        info = pic.jfnk_step(E, dt, rtol=rtol, jacobian=jac)
+        assert info["converged"], info
+    # exact sub-steps / crossings of ONE mover pass from the state the timed steps start at
+    # (counting build; the timed passes run the fast build, which counts in groups of 4 rounds)
+    pic.set_flags(flags | B.PIC_FLAG_DIAG)
+    pic.move_accumulate(E, E, dt)
+    exact = pic.get_stats()
+    pic.set_flags(flags)
+    if not explicit_steps and args.min_seconds > 0:
+        t0 = time.perf_counter()
+        pic.jfnk_step(E, dt, rtol=rtol, jacobian=jac)
+        args.steps = max(args.steps, min(2000, int(math.ceil(args.min_seconds / max(time.perf_counter() - t0, 1e-4)))))
+    e_start = energy()
+    sampler = ClockSampler(local_rank)
+    hist, kms, launches0 = [], [], pic.get_stats()["n_launches"]
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        info = pic.jfnk_step(E, dt, rtol=rtol, jacobian=jac)
+        hist.append(info)
+    e1.record()
+    barrier()
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    st = pic.get_stats()
+    launches = st["n_launches"] - launches0
+    assert all(h["converged"] for h in hist), hist
+    e_end = energy()
+    rho = pic.rho(B.PIC_STATE_N)
+    gauss = float(np.linalg.norm((np.roll(E, -1) - E) / dx - rho) / max(np.linalg.norm(rho), 1e-300))
+    gauss_abs = float(np.max(np.abs((np.roll(E, -1) - E) / dx - rho)))
+    for _ in range(3):                                   # the mover pass alone (library events)
+        pic.move_accumulate(E, E, dt)
+        kms.append(pic.get_stats()["last_move_ms"])
+    k_ms = float(np.mean(kms))
+    calls = float(np.sum([h["mover_calls"] for h in hist]))
+    calls_resid = float(np.sum([h["mover_calls_resid"] for h in hist]))
+    n_sub, n_cross = exact["n_sub"], exact["n_cross"]
+    ms, wall, tot_sub, tot_cross = replicas.aggregate(ms, wall, n_sub * calls, n_cross * calls, device="cuda")
+    if rank != 0:
+        pic.close()
+        return
+    props = torch.cuda.get_device_properties(local_rank)
+    sms = props.multi_processor_count
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:  # noqa: BLE001
+        peaks = {}
+    sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    lanes = 128 if args.precision == "fp32" else 64
+    peak_gops = sms * lanes * 2 * sm_max_mhz * 1e-3
+    ops_per_pass = OPS_INCELL * (n_sub - n_cross) + OPS_CROSS * n_cross
+    achieved = ops_per_pass / (k_ms * 1e-3) * 1e-9
+    value = tot_sub / (ms * 1e-3)
+    steps = args.steps
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": ms / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if args.precision == "fp32" else "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: ion acoustic wave, {ng} cells, "
+                               f"{'+'.join(str(n) for n in pic.n)} particles/GPU, dt={dt}, full implicit step",
+                   "precision": args.precision + (" residual + fp32 J w (defect correction)" if jac else ""),
+                   "cn_mode": args.cn_mode, "jfnk_rtol": rtol,
+                   "substeps_per_particle_per_pass": n_sub / max(n_p, 1),
+                   "crossing_fraction": n_cross / max(n_sub, 1),
+                   "substep_count": "one counting-build pass from the state the timed steps start at, x mover passes",
+                   "l2": "particle state %.0f MB/GPU (fits the 126 MB L2 only for cfg1 in fp32); every "
+                         "pass rereads all of it" % (n_p * (12 if args.precision == "fp32" else 20) * 1e-6),
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "implicit_step": {
+            "ms_per_step": ms / steps, "wall_ms_per_step": 1e3 * wall / steps,
+            "newton_its_mean": float(np.mean([h["newton_its"] for h in hist])),
+            "gmres_its_mean": float(np.mean([h["gmres_its"] for h in hist])),
+            "mover_passes_mean": calls / steps, "mover_passes_fp64_mean": calls_resid / steps if jac else None,
+            "mover_ms_per_pass": k_ms,
+            "mover_share_of_step": None if jac else k_ms * calls / steps / (ms / steps),
+            "energy_rel_change_per_step": abs(e_end - e_start) / e_start / steps,
+            "energy_rel_change_total": (e_end - e_start) / e_start,
+            "gauss_residual_rel": gauss, "gauss_residual_max_abs": gauss_abs,
+            "resid_last": hist[-1]["resid"], "resid0_last": hist[-1]["resid0"]},
+        "gop_per_s_model": value * ops_per_pass / max(n_sub, 1) * 1e-9,
+        "clocks": clocks,
+        "e2e": {"value": value, "unit": UNIT,
+                "h2d_bytes_per_step": int(calls / steps * ng * 8 + ng * 8),
+                "d2h_bytes_per_step": int(calls / steps * ng * 8),
+                "note": "the timed value already passes host E in and the residual out on every mover pass"},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_gops, "unit": "GOp/s",
+                     "frac": achieved / peak_gops, "traffic": None,
+                     "kernel": pic.last_kernel() + " (all species of one pass)", "kernel_ms": k_ms,
+                     "ops_per_launch": ops_per_pass,
+                     "convention": "paper's op count (P:94-105), algorithmic table of DESIGN.md 6; NOT flops",
+                     "peak_source": "derived: SMs x lanes x 2 x sm_max_mhz (DESIGN.md 6)",
+                     "note": "passes of 1-4 M particles are latency-bound (two launches of 0.1 ms)"},
+    }
+    pic.close()
+    if jac is not None:
+        jac.close()
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=0,
+                    help="timed steps; 0 = 10, raised until the timed region lasts --min-seconds")
+    ap.add_argument("--min-seconds", type=float, default=2.0,
+                    help="without --steps: time enough steps for a region this long (clock samples)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg2", "cfg3"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"],
+                    help="BASELINE.json configs[k]; cfg1 / cfg4 time the full implicit step (JFNK)")
+    ap.add_argument("--rtol", type=float, default=0.0, help="cfg1/cfg4: nonlinear tolerance (0 = per precision)")
+    ap.add_argument("--defect-correction", action="store_true",
+                    help="cfg1/cfg4 with --precision fp64: fp32 Jacobian-vector products (P:325-331)")
     ap.add_argument("--n", type=int, default=0, help="override the particle count (debug)")
-    ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
+    ap.add_argument("--precision", default=None, choices=["fp32", "fp64"],
+                    help="default: fp32 (cfg1: fp64, BASELINE.json configs[1])")
     ap.add_argument("--cn-mode", default="direct", choices=["direct", "picard"])
     ap.add_argument("--seed", type=int, default=W.DEFAULT_SEED)
     ap.add_argument("--cpu-sample", type=int, default=1 << 22)
     ap.add_argument("--ref-sample", type=int, default=1 << 19)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vsort", action="store_true", help="bin by cell only (default: phase-space cell)")
-    ap.add_argument("--fp64-n", type=int, default=20_000_000,
+    ap.add_argument("--fp64-n", type=int, default=-1,
                     help="with --precision fp32: also time the fp64 mover on the first N particles of "
-                         "the same workload and report it under 'fp64' (0 = skip)")
+                         "the same workload and report it under 'fp64' (-1 = all of them, 0 = skip)")
     ap.add_argument("--microbench", action="store_true",
                     help="only run the P:86 instruction micro-benchmarks (pic_microbench) and print them")
     ap.add_argument("--histogram", action="store_true",
@@ -191,15 +387,35 @@ def main():
                          "(BASELINE.json configs[3]); keeps 8 B per particle of counters")
     ap.add_argument("--one-per-lane", action="store_true",
                     help="fp32: the one-particle-per-lane kernel instead of the packed two-per-lane one")
+    ap.add_argument("--strided", action="store_true",
+                    help="the paper's particle order (Eq. 15): consecutive particles in consecutive cells")
+    ap.add_argument("--per-visit", action="store_true",
+                    help="deposit per cell visit with shared fp64 atomics (P:222) instead of the end-point form")
     ap.add_argument("--vp", action="store_true",
                     help="Vlasov-Poisson variant of the mover: orbits without the current deposit (P:281)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    if args.precision is None:
+        args.precision = "fp64" if args.workload == "cfg1" else "fp32"
+    explicit_steps = args.steps > 0
+    if not explicit_steps:
+        args.steps = 10
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # --gpus N outside torchrun: launch the N replicas ourselves (one rank per GPU)
+        import subprocess
+        port = 29500 + os.getpid() % 2000
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+               f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1", "--master-port",
+               str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    if args.gpus != world and "WORLD_SIZE" in os.environ and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; using the launcher's {world}",
+              file=sys.stderr)
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
@@ -228,6 +444,10 @@ def main():
                               "fp64_gflops_measured_dfma": 2 * mb["dfma"]["thread_gops"]}), flush=True)
         return
 
+    if args.workload in ("cfg1", "cfg4"):
+        run_iaw(args, rank, world, local_rank, explicit_steps)
+        return
+
     # replicas only: every rank runs its own copy of the workload with its own seed
     from paper_1111_5295_b200 import replicas as _rep
     cfg = _workload(args.workload, args.n, _rep.rank_seed(args.seed, rank))
@@ -239,6 +459,10 @@ def main():
         flags |= B.PIC_FLAG_NO_DEPOSIT
     if args.one_per_lane:
         flags |= B.PIC_FLAG_ONE_PER_LANE
+    if args.strided:
+        flags |= B.PIC_FLAG_STRIDED
+    if args.per_visit:
+        flags |= B.PIC_FLAG_DEPOSIT_PER_VISIT
     init_flags = flags | (B.PIC_FLAG_COUNTS if args.histogram else 0)   # allocates the counters
     pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision=args.precision,
                 cn_mode=args.cn_mode, flags=init_flags, stream=stream)
@@ -278,6 +502,16 @@ def main():
     for _ in range(args.warmup):
         pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
     torch.cuda.synchronize()
+    if not explicit_steps and args.min_seconds > 0:
+        # enough steps for a timed region of --min-seconds (the clock record needs samples under
+        # load); every rank takes the same count
+        w_ms = max(pic.get_stats()["last_move_ms"], 1e-3)
+        want = int(math.ceil(args.min_seconds * 1e3 / w_ms))
+        if world > 1:
+            t = torch.tensor([want], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            want = int(t.item())
+        args.steps = max(args.steps, min(want, 100000))
     st0 = pic.get_stats()
     sampler = ClockSampler(local_rank)
     barrier()
@@ -309,6 +543,14 @@ def main():
         pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
         kms.append(pic.get_stats()["last_move_ms"])
     k_ms = float(np.mean(kms))
+    # ---- pic_commit (accept state n+1, re-bin by phase-space cell): once per time step, never per
+    # residual; timed last because it replaces state n
+    c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    c0.record()
+    pic.commit()
+    c1.record()
+    torch.cuda.synchronize()
+    commit_ms = c0.elapsed_time(c1)
 
     from paper_1111_5295_b200 import replicas
     ms, e2e_s, tot_sub, tot_cross = replicas.aggregate(ms, e2e_s, n_sub, n_cross, device="cuda")
@@ -335,6 +577,7 @@ def main():
     ops_per_launch = OPS_INCELL * (n_sub - n_cross) + OPS_CROSS * n_cross
     kernel_name = pic.last_kernel()        # the kernel the timed launches ran (library's word)
     achieved = ops_per_launch / (k_ms * 1e-3) * 1e-9
+    executed = NCU_EXECUTED_OPS.get((args.workload, n_p, args.precision, kernel_name))
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -343,12 +586,17 @@ def main():
         "config": {"workload": f"{args.workload}: {ng} cells, {n_p} particles/GPU, dt={dt}",
                    "precision": args.precision, "cn_mode": args.cn_mode,
                    "variant": "VP (no current deposit, P:281)" if args.vp else "VA (orbit-averaged current)",
-                   "binning": "cell" if args.no_vsort else "phase-space cell: cell + offset class + velocity class (P:242-250)",
+                   "binning": "cell" if args.no_vsort else
+                              ("strided (P:244-250, Eq. 15): velocity class + offset class + cell" if args.strided
+                               else "phase-space cell: cell + offset class + velocity class (P:242-250)"),
+                   "deposit": "per cell visit, shared fp64 atomics (P:222)" if args.per_visit else "end-point form",
                    "substeps_per_particle": n_sub / max(n_p, 1),
                    "crossing_fraction": n_cross / max(n_sub, 1),
                    "l2": "inputs larger than L2 (particle state %.0f MB/GPU)" % (n_p * 12e-6),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "gop_per_s_model": value * ops_per_launch / max(n_sub, 1) * 1e-9,
+        "commit": {"ms": commit_ms, "note": "pic_commit after one step: swap + re-binning of all particles, "
+                                            "once per time step (P:250); a time step is 13-33 mover passes"},
         "clocks": clocks,
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 2 * ng * 8,
                 "d2h_bytes_per_step": ng * 8},
@@ -358,6 +606,16 @@ def main():
                      "traffic": NCU_TRAFFIC_BYTES.get((args.workload, n_p, args.precision)),
                      "traffic_unit": "bytes per launch (ncu dram read+write); algorithmic %d"
                                      % (n_p * (24 if args.precision == "fp32" else 40)),
+                     "traffic_source": NCU_TRAFFIC_SOURCE,
+                     "convention": "paper's op count (P:94-105): every FP/int/SF thread-operation 1, "
+                                   "FMA 2, from the algorithmic table of DESIGN.md 6; NOT flops",
+                     "frac_executed": (executed[0] * n_sub / (k_ms * 1e-3) * 1e-9 / peak_gops
+                                       if executed else None),
+                     "frac_fp_only": (executed[1] * n_sub / (k_ms * 1e-3) * 1e-9 / peak_gops
+                                      if executed else None),
+                     "executed_source": "thread-operations per sub-step from the SASS counters of "
+                                        + NCU_TRAFFIC_SOURCE + ": all instructions by the paper's "
+                                        "convention / floating-point arithmetic only",
                      "kernel": kernel_name, "kernel_ms": k_ms,
                      "ops_per_launch": ops_per_launch,
                      "peak_source": "derived: SMs x lanes x 2 x sm_max_mhz (DESIGN.md 6)",
@@ -369,8 +627,8 @@ def main():
     pic = None
     # ---- BASELINE.json's metric names both precisions: the fp64 instantiation of the mover on
     # the first fp64_n particles of the same workload (same fields, same dt), kernel-timed
-    if args.precision == "fp32" and args.fp64_n > 0 and not args.vp:
-        n64 = min(args.fp64_n, n_p)
+    if args.precision == "fp32" and args.fp64_n != 0 and not args.vp and args.workload in ("cfg2", "cfg3"):
+        n64 = n_p if args.fp64_n < 0 else min(args.fp64_n, n_p)
         sp64 = dict(sp, x=sp["x"][:n64], v=sp["v"][:n64], w_q=sp["w_q"] * n_p / n64)
         p64 = B.Pic(cfg["n_cells"], cfg["length"], [sp64], precision="fp64", cn_mode=args.cn_mode,
                     flags=(0 if args.no_vsort else B.PIC_FLAG_VSORT) | B.PIC_FLAG_DIAG, stream=stream)

@@ -55,6 +55,9 @@ enum {
   PIC_FLAG_ONE_PER_LANE = 64, /* fp32 only: run the one-particle-per-lane kernel also where the
                               default two-particles-per-lane packed-FP32 kernel (FFMA2) applies;
                               both give bit-identical orbits (A/B timing, tests)               */
+  PIC_FLAG_STRIDED = 256,  /* with PIC_FLAG_VSORT: the paper's own particle order (Eq. 15):
+                              consecutive particles lie in consecutive CELLS and share a velocity
+                              class, instead of sharing a cell (A/B of S8(f) #3; same results)   */
   PIC_FLAG_EXACT_TIME = 128, /* fp32 only: exact accounting of the time used by the sub-steps
                               (fp64 checkpoints of the remaining time, D:5) instead of a plain
                               fp32 `r -= dtau`, whose rounding random-walks to ~ulp(dt) sqrt(n_sub) */

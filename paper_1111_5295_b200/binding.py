@@ -23,6 +23,7 @@ PIC_FLAG_DEPOSIT_PER_VISIT = 16
 PIC_FLAG_NO_DEPOSIT = 32
 PIC_FLAG_ONE_PER_LANE = 64
 PIC_FLAG_EXACT_TIME = 128
+PIC_FLAG_STRIDED = 256
 PIC_ERR_SUBSTEP_CAP = -4
 
 EXPORTS = ["pic_init", "pic_move_accumulate", "pic_set_step", "pic_residual", "pic_commit",

@@ -58,7 +58,9 @@ int from_device(pic_handle* h, const double* dsrc, double* dst) {
   return PIC_OK;
 }
 
-VKey key_of(const SpeciesState& S) { return VKey{S.nx, S.nv, S.vmean, S.vinv}; }
+VKey key_of(const pic_handle* h, const SpeciesState& S) {
+  return VKey{S.nx, S.nv, S.vmean, S.vinv, S.strided ? h->grid.n_cells : 0, 0};
+}
 
 // exclusive scan of d_hist[0..nk) (three small kernels)
 int scan_hist(pic_handle* h, long long nk) {
@@ -115,6 +117,20 @@ int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double*
 #ifndef PIC_NVMAX
 #define PIC_NVMAX 1024
 #endif
+    const bool strided = (h->params.flags & PIC_FLAG_STRIDED) != 0;
+    if (strided) {
+      // about one particle per key: 256 velocity rows (fewer for thin species), the rest of the
+      // particles of a cell spread over offset classes
+#ifndef PIC_STRIDE_NV
+#define PIC_STRIDE_NV 256
+#endif
+#ifndef PIC_STRIDE_PPK
+#define PIC_STRIDE_PPK 1
+#endif
+      nx = 1;
+      while (nv < PIC_STRIDE_NV && (double)nv * 2 * 2 <= ppc) nv *= 2;
+      while (nx < 4096 && (double)nx * 2 * nv * PIC_STRIDE_PPK <= ppc) nx *= 2;
+    } else
     while (nv < PIC_NVMAX && (double)nx * nv * 2 * PIC_PPK <= ppc) nv *= 2;
     while (nx > 1 && (long long)ng * nx * nv > h->n_keys) nx /= 2;
     while (nv > 1 && (long long)ng * nx * nv > h->n_keys) nv /= 2;
@@ -123,9 +139,10 @@ int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double*
       S.nv = nv;
       S.vmean = mean;
       S.vinv = (double)nv / (8.0 * std::sqrt(var));
+      S.strided = strided;
     }
   }
-  const VKey vk = key_of(S);
+  const VKey vk = key_of(h, S);
   const long long nk = (long long)ng * S.nx * S.nv;
   // stage 1: cell/xi/v in input order into buffer 1-b, histogram over the sort keys
   PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (nk + 1), h->stream));
@@ -146,7 +163,7 @@ int rebin_species(pic_handle* h, SpeciesState& S) {
   // state n+1 lives in buffer 1-cur; scatter it, binned, into buffer cur (old state n is dead).
   const int32_t ng = h->grid.n_cells;
   const int src = 1 - h->cur, dst = h->cur;
-  const VKey vk = key_of(S);
+  const VKey vk = key_of(h, S);
   const long long nk = (long long)ng * S.nx * S.nv;
   if (nk > h->n_keys) return set_err(h, PIC_ERR_STATE, "rebin: sort key larger than the binning scratch");
   PIC_CUDA(h, cudaMemsetAsync(h->d_hist, 0, sizeof(int32_t) * (nk + 1), h->stream));
@@ -413,7 +430,7 @@ int pic_copy_state(pic_handle* dst, pic_handle* src) {
     }
     PIC_CUDA(dst, cudaMemcpyAsync(Bs.cell[b], A.cell[a], sizeof(int32_t) * A.n, cudaMemcpyDeviceToDevice, dst->stream));
     PIC_CUDA(dst, cudaMemcpyAsync(Bs.id[b], A.id[a], sizeof(uint32_t) * A.n, cudaMemcpyDeviceToDevice, dst->stream));
-    Bs.nx = A.nx; Bs.nv = A.nv; Bs.vmean = A.vmean; Bs.vinv = A.vinv;
+    Bs.nx = A.nx; Bs.nv = A.nv; Bs.vmean = A.vmean; Bs.vinv = A.vinv; Bs.strided = A.strided;
   }
   PIC_CUDA(dst, cudaGetLastError());
   dst->have_np1 = false;

@@ -22,6 +22,7 @@ struct SpeciesState {
   uint32_t* ncross = nullptr;
   int32_t nx = 1, nv = 1;                 // offset / velocity classes of the sort key (1 = cell only)
   double vmean = 0, vinv = 0;
+  bool strided = false;                   // PIC_FLAG_STRIDED: (v class, offset class, cell) order
   int grid_blocks = 0;                    // mover launch shape for this species
   int grid_blocks2 = 0;                   // same for the two-per-lane fp32 kernel (0 = not usable)
   int last_blocks = 0;                    // blocks (= rows of `partial`) of the last launch

@@ -12,15 +12,25 @@ namespace picb200 {
 // that neighbours in memory share the cell and the offset class and have adjacent velocities.
 // Lanes of a warp then start almost the same orbit: same sub-step sequence, crossings in the same
 // round, orbit ends in the same round.
+//
+// PIC_FLAG_STRIDED orders the same three sub-keys the other way round, (velocity class, offset
+// class, cell): the paper's own layout (Eq. 15), in which consecutive threads hold
+// particles of CONSECUTIVE cells with similar velocities (made for its per-warp atomic deposits,
+// where lanes sharing a cell collide).  With about one particle per key the offset class plays
+// the part of the paper's index p of a particle inside its phase-space cell.  Kept for the A/B
+// of SURVEY 8(f) #3 (profiles/r2_strided_layout.md).
 struct VKey {
   int32_t nx, nv;
   double vmean, vinv;   // vinv = nv / (8 sigma)
+  int32_t n_cells;      // > 0: strided order (v class, offset class, cell); 0: cell-major order
+  int32_t pad_;
 };
 __device__ __forceinline__ int32_t sort_key(const VKey& k, int32_t cell, double xi, double v) {
   if (k.nv <= 1 && k.nx <= 1) return cell;
   const double t = (v - k.vmean) * k.vinv + 0.5 * k.nv;
   const int32_t b = (int32_t)fmin(fmax(t, 0.0), (double)(k.nv - 1));
   const int32_t xb = min((int32_t)(xi * k.nx), k.nx - 1);
+  if (k.n_cells > 0) return (b * k.nx + xb) * k.n_cells + cell;
   return (cell * k.nx + xb) * k.nv + b;
 }
 

@@ -121,6 +121,25 @@ def test_vsort_parity_and_commit(G, oracle, precision):
     pic.close()
 
 
+# ---- the paper's own particle order (Eq. 15): consecutive particles in consecutive cells ----------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("per_visit", [False, True])
+def test_strided_layout_parity(G, oracle, precision, per_visit):
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config2(n=150_001)
+    extra = B.PIC_FLAG_VSORT | B.PIC_FLAG_STRIDED | (B.PIC_FLAG_DEPOSIT_PER_VISIT if per_visit else 0)
+    m = G.parity(oracle, cfg, precision, extra_flags=extra, fast=not per_visit)
+    _report(f"cfg2/150k {precision} strided per_visit={per_visit}", m)
+    G.assert_parity(m, precision)
+    pic = m["gpu"]["pic"]
+    before = pic.get_particles(0, B.PIC_STATE_NP1)
+    pic.commit()
+    after = pic.get_particles(0, B.PIC_STATE_N)
+    for k in ("x", "v", "cell", "xi"):
+        assert np.array_equal(before[k], after[k]), k
+    pic.close()
+
+
 # ---- the fast build (no per-sub-step counting) computes the same orbits as the counting build --
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_fast_build_matches_counting_build(G, precision):
