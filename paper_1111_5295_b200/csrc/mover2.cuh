@@ -99,19 +99,6 @@ __device__ __forceinline__ void cross2(const MoverArgs<float>& a, const float4* 
 
 // One sub-step (O3-O8) of both slots.  A parked or empty slot has r = 0, so dtau = 0 and the
 // tentative step reproduces (xi, u) bit for bit and is accepted (no per-slot guard).
-// Crossing schedule (PIC_DEFER): g = index of the round inside its group of kGroup.  0 = every
-// round may cross (a lane-divergent branch).  Otherwise a slot whose tentative step left its cell
-// is HELD in the rounds that may not cross: it keeps (xi, u), uses no time, and recomputes the
-// same tentative step in the next round -- bit-identical orbits, but the crossing blocks run in
-// fewer rounds with more lanes each (lanes of a phase-space-binned warp reach the face within a
-// round or two of one another).
-#ifndef PIC_DEFER
-#define PIC_DEFER 0
-#endif
-#ifndef PIC_DEFER_T
-#define PIC_DEFER_T 24
-#endif
-template <int G>
 __device__ __forceinline__ void substep2(const MoverArgs<float>& a, const float4* __restrict__ sC,
                                          Lane2& p) {
   const float2 half2 = make_float2(0.5f, 0.5f), one2 = make_float2(1.0f, 1.0f),
@@ -145,77 +132,11 @@ __device__ __forceinline__ void substep2(const MoverArgs<float>& a, const float4
   float2 used = dtau;
   // ---- O6 / O7: accept both (inclusive, A-5), or truncate the slots that left their cell
   const bool ok0 = in_unit<float>(nxi.x), ok1 = in_unit<float>(nxi.y);
-#if PIC_DEFER == 0
-  if (!(ok0 && ok1)) {
-    if (!ok0) cross2<0>(a, sC, p, A, dtau, nxi, nu, used);
-    if (!ok1) cross2<1>(a, sC, p, A, dtau, nxi, nu, used);
-  }
-#elif PIC_DEFER == 5
-  // as 0, behind a warp-uniform vote
+  // (behind a warp-uniform vote: the divergent per-slot blocks then sit inside a uniform branch)
   if (__any_sync(kFull, !(ok0 && ok1))) {
     if (!ok0) cross2<0>(a, sC, p, A, dtau, nxi, nu, used);
     if (!ok1) cross2<1>(a, sC, p, A, dtau, nxi, nu, used);
   }
-#elif PIC_DEFER == 1
-  // static schedule: crossings in the odd rounds of a group only
-  if (!(ok0 && ok1)) {
-    if (G & 1) {
-      if (!ok0) cross2<0>(a, sC, p, A, dtau, nxi, nu, used);
-      if (!ok1) cross2<1>(a, sC, p, A, dtau, nxi, nu, used);
-    } else {
-      if (!ok0) { nxi.x = p.xi.x; nu.x = p.u.x; used.x = 0.0f; }
-      if (!ok1) { nxi.y = p.xi.y; nu.y = p.u.y; used.y = 0.0f; }
-    }
-  }
-#elif PIC_DEFER == 2
-  // last round of a group always crosses; the others only once PIC_DEFER_T slots are waiting
-  {
-    const unsigned m0 = __ballot_sync(kFull, !ok0), m1 = __ballot_sync(kFull, !ok1);
-    if (m0 | m1) {
-      const bool go = (G == kGroup - 1) || (__popc(m0) + __popc(m1) >= PIC_DEFER_T);
-      if (go) {
-        if (!ok0) cross2<0>(a, sC, p, A, dtau, nxi, nu, used);
-        if (!ok1) cross2<1>(a, sC, p, A, dtau, nxi, nu, used);
-      } else {
-        if (!ok0) { nxi.x = p.xi.x; nu.x = p.u.x; used.x = 0.0f; }
-        if (!ok1) { nxi.y = p.xi.y; nu.y = p.u.y; used.y = 0.0f; }
-      }
-    }
-  }
-#elif PIC_DEFER == 4
-  // the last round of a group always crosses, round 1 once PIC_DEFER_T slots wait, 0 and 2 never
-  {
-    bool go = G == 3;
-    if (G == 1) {
-      const unsigned m0 = __ballot_sync(kFull, !ok0), m1 = __ballot_sync(kFull, !ok1);
-      go = __popc(m0) + __popc(m1) >= PIC_DEFER_T;
-    }
-    if (!(ok0 && ok1)) {
-      if (go) {
-        if (!ok0) cross2<0>(a, sC, p, A, dtau, nxi, nu, used);
-        if (!ok1) cross2<1>(a, sC, p, A, dtau, nxi, nu, used);
-      } else {
-        if (!ok0) { nxi.x = p.xi.x; nu.x = p.u.x; used.x = 0.0f; }
-        if (!ok1) { nxi.y = p.xi.y; nu.y = p.u.y; used.y = 0.0f; }
-      }
-    }
-  }
-#elif PIC_DEFER == 3
-  // odd rounds always cross; even rounds only once PIC_DEFER_T slots are waiting
-  {
-    const unsigned m0 = __ballot_sync(kFull, !ok0), m1 = __ballot_sync(kFull, !ok1);
-    if (m0 | m1) {
-      const bool go = (G & 1) || (__popc(m0) + __popc(m1) >= PIC_DEFER_T);
-      if (go) {
-        if (!ok0) cross2<0>(a, sC, p, A, dtau, nxi, nu, used);
-        if (!ok1) cross2<1>(a, sC, p, A, dtau, nxi, nu, used);
-      } else {
-        if (!ok0) { nxi.x = p.xi.x; nu.x = p.u.x; used.x = 0.0f; }
-        if (!ok1) { nxi.y = p.xi.y; nu.y = p.u.y; used.y = 0.0f; }
-      }
-    }
-  }
-#endif
   p.xi = nxi;
   p.u = nu;
   p.r = __ffma2_rn(used, mone2, p.r);
@@ -358,11 +279,8 @@ mover2_kernel(const MoverArgs<float> a) {
     for (int j = 0; j < kInner / kGroup; ++j) {
       if (p.r.x > 0.0f) p.ns[0] += kGroup;
       if (p.r.y > 0.0f) p.ns[1] += kGroup;
-      static_assert(kGroup == 4, "the rounds of a group are written out");
-      substep2<0>(a, sC, p);
-      substep2<1>(a, sC, p);
-      substep2<2>(a, sC, p);
-      substep2<3>(a, sC, p);
+#pragma unroll
+      for (int g = 0; g < kGroup; ++g) substep2(a, sC, p);
       if (!__any_sync(kFull, p.r.x > 0.0f || p.r.y > 0.0f)) break;
     }
   }
