@@ -165,3 +165,95 @@ def test_defect_correction_matches_fp64(oracle):
     assert abs(e1 - e0) / e0 < 1e-8
     for p in (ref, h64, h32):
         p.close()
+
+
+def test_cfg1_full_size_ten_steps(oracle):
+    """BASELINE.json configs[1] as stated: 256 cells, 2 x 512,000 particles, dt = 1, host fp64
+    JFNK at nonlinear relative tolerance 1e-8 around the fp64 GPU mover, 10 steps.  At every step
+    the ORACLE's residual at the converged field, from the same state n, must be as small as the
+    solver's; total energy is conserved to the nonlinear tolerance."""
+    from paper_1111_5295_b200 import binding as B
+    from paper_1111_5295_b200.iaw import gauss_field
+    import gpu_helpers as G
+    cfg = W.config1()
+    ng, L, dt = cfg["n_cells"], cfg["length"], cfg["dt"]
+    dx = L / ng
+    pic = B.Pic(ng, L, cfg["species"], precision="fp64", cn_mode="direct", flags=B.PIC_FLAG_VSORT)
+    E = gauss_field(pic.rho(B.PIC_STATE_N), dx)
+
+    def energy():
+        return float(pic.kinetic_energy(B.PIC_STATE_N).sum() + 0.5 * dx * np.sum(E * E))
+
+    e0 = energy()
+    for step in range(10):
+        En = E.copy()
+        before = [pic.get_particles(j, B.PIC_STATE_N) for j in range(2)]
+        info = pic.jfnk_step(E, dt, rtol=1e-8)
+        assert info["rc"] == 0 and info["converged"] == 1, info
+        state = [(b["cell"], b["xi"] * dx, b["v"]) for b in before]
+        ref = G.oracle_run(oracle, dict(cfg, E_n=En, E_np1=E),
+                           oracle.make_params(cn_mode=oracle.DIRECT), state=state)
+        Ro = float(np.linalg.norm(oracle.residual(En, E, dt, ref["jbar"])))
+        print(f"[cfg1] step {step + 1}: newton={info['newton_its']} gmres={info['gmres_its']} "
+              f"passes={info['mover_calls']} |R0|={info['resid0']:.2e} |R|={info['resid']:.2e} "
+              f"oracle |R|={Ro:.2e} dE/E={(energy() - e0) / e0:+.2e}")
+        assert Ro <= 2e-8 * info["resid0"]
+        rho = pic.rho(B.PIC_STATE_N)
+        assert np.linalg.norm((np.roll(E, -1) - E) / dx - rho) <= 1e-6 * np.linalg.norm(rho)
+    assert abs(energy() - e0) / e0 < 1e-9
+    pic.close()
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_cfg3_full_size_invariants(oracle, precision):
+    """BASELINE.json configs[3] at full size (2e7 particles) in the launch configuration the bench
+    times: properties that hold at any size -- per-cell continuity with rho by the oracle from the
+    kernel's own (cell, xi), the energy identity, no sub-step cap -- plus sampled orbits against
+    the oracle one by one (fp64: north_star's bars; fp32: the derived bars of DESIGN.md 2)."""
+    import torch
+    from paper_1111_5295_b200 import binding as B
+    import gpu_helpers as G
+    from helpers import ulp_response
+    cfg = W.config3()
+    sp = cfg["species"][0]
+    n, ng, dt = sp["x"].shape[0], cfg["n_cells"], cfg["dt"]
+    dx = cfg["length"] / ng
+    pic = B.Pic(ng, cfg["length"], [sp], precision=precision, flags=B.PIC_FLAG_VSORT | B.PIC_FLAG_COUNTS,
+                stream=torch.cuda.current_stream().cuda_stream)
+    pic.move_accumulate(cfg["E_n"], cfg["E_np1"], dt)                 # counting build
+    st = pic.get_stats()
+    assert st["n_substep_cap"] == 0 and st["n_sub"] > 500 * n
+    nsub = torch.empty(n, dtype=torch.int32, device="cuda")
+    ncross = torch.empty(n, dtype=torch.int32, device="cuda")
+    pic._chk(pic._L.pic_get_counts(pic._h, C.c_int(0), B._ptr(nsub), B._ptr(ncross)))
+    pic.set_flags(B.PIC_FLAG_VSORT)                                   # the timed (fast) build
+    jbar = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], dt)
+    assert pic.last_kernel() == ("mover2_kernel" if precision == "fp32" else "mover_kernel")
+    c0, x0, v0 = _device_state(pic, B, torch, B.PIC_STATE_N)
+    c1, x1, v1 = _device_state(pic, B, torch, B.PIC_STATE_NP1)
+    rho0 = oracle.rho(ng, cfg["length"], sp["w_q"], c0.cpu().numpy(), x0.cpu().numpy() * dx)
+    rho1 = oracle.rho(ng, cfg["length"], sp["w_q"], c1.cpu().numpy(), x1.cpu().numpy() * dx)
+    div = dt * (np.roll(jbar, -1) - jbar) / dx
+    cont = np.linalg.norm(rho1 - rho0 + div) / np.linalg.norm(div)
+    dK = pic.kinetic_energy(B.PIC_STATE_NP1)[0] - pic.kinetic_energy(B.PIC_STATE_N)[0]
+    work = dt * dx * np.sum(jbar * 0.5 * (cfg["E_n"] + cfg["E_np1"]))
+    print(f"[cfg3 full] {precision}: continuity {cont:.2e} energy identity {(dK - work) / abs(work):.2e}")
+    assert cont <= (1e-10 if precision == "fp64" else 1e-5)
+    assert abs(dK - work) <= (1e-9 if precision == "fp64" else 1e-3) * abs(work)
+    idx = torch.from_numpy(np.sort(np.random.default_rng(4).choice(n, 1 << 13, replace=False))).cuda()
+    h = lambda t: t[idx].cpu().numpy()
+    r = oracle.move_accumulate(ng, cfg["length"], sp["q_over_m"], sp["w_q"], h(c0), h(x0) * dx, h(v0),
+                               cfg["E_n"], cfg["E_np1"], dt, oracle.make_params(cn_mode=oracle.DIRECT))
+    same = (r["n_sub"] == h(nsub).astype(np.uint32)) & (r["n_cross"] == h(ncross).astype(np.uint32)) \
+        & (r["cell"] == h(c1))
+    xg, xr = (h(c1) + h(x1)) * dx, r["cell"] * dx + r["s"]
+    ex = np.linalg.norm(G.periodic_dist(xg[same], xr[same], cfg["length"])) / np.linalg.norm(xr[same])
+    ev = G.rel_l2(h(v1)[same], r["v"][same])
+    print(f"[cfg3 full] {precision}: sampled 8192 of {n}: x={ex:.2e} v={ev:.2e} flips={int((~same).sum())}")
+    if precision == "fp64":
+        assert ex <= 1e-10 and ev <= 1e-10 and (~same).sum() <= 8
+    else:
+        u = ulp_response(oracle, W.config3(n=20_011))
+        k = 3.0 * math.sqrt(u["n_sub_mean"])
+        assert ex <= k * u["x"] and ev <= k * u["v"] and (~same).sum() <= 0.05 * same.size
+    pic.close()
