@@ -237,6 +237,14 @@ const char* pic_last_kernel(const pic_handle* h);
  * stream and synchronises it. */
 int pic_microbench(int which, int iters, double* thread_gops, int* n_sm);
 
+/* pic_debug_bounds — the debug build libpic_b200_check.so (-DPIC_BOUNDS_CHECK=1) checks every
+ * shared- and global-memory index its kernels derive from particle data (cell indices, sort
+ * keys, scatter destinations, queue positions) and counts the ones out of range (D:7; the pool's
+ * compute-sanitizer is closed).  *violations receives that count since the library was loaded
+ * (synchronises the device), or -1 from the production build, whose checks compile to nothing.
+ * self_test != 0 first provokes exactly one violation, to show that the counter works. */
+int pic_debug_bounds(int64_t* violations, int self_test);
+
 /* Library/device identification for logs: fills buf with e.g. "pic_b200 sm_100a ...". */
 int pic_version(char* buf, int buflen);
 

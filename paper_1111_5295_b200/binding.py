@@ -29,7 +29,8 @@ PIC_ERR_SUBSTEP_CAP = -4
 EXPORTS = ["pic_init", "pic_move_accumulate", "pic_set_step", "pic_residual", "pic_commit",
            "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_set_flags",
            "pic_kinetic_energy", "pic_rho", "pic_jfnk_step", "pic_jfnk_step_dc",
-           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_last_kernel", "pic_version", "pic_count_histogram", "pic_microbench"]
+           "pic_copy_state", "pic_destroy", "pic_last_error", "pic_last_kernel", "pic_version", "pic_count_histogram", "pic_microbench",
+           "pic_debug_bounds"]
 
 
 class PicGrid(C.Structure):
@@ -87,10 +88,12 @@ def lib_path():
 
 
 def load():
-    """dlopen libpic_b200.so (building it first if the sources are newer).  Raises if absent."""
+    """dlopen libpic_b200.so (building it first if the sources are newer).  Raises if absent.
+    PIC_B200_CHECK=1 in the environment selects the bounds-checked debug build
+    (libpic_b200_check.so, see pic_debug_bounds)."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        path = _build.build(check=os.environ.get("PIC_B200_CHECK", "0") == "1")
         if not os.path.exists(path):
             raise RuntimeError(f"CUDA extension missing: {path} (run __graft_entry__.build())")
         L = C.CDLL(path)
@@ -143,6 +146,15 @@ def microbench(iters=20000, sm_mhz=1965.0):
         out[name] = {"thread_gops": gops.value,
                      "per_clk_per_sm": gops.value * 1e3 / (sms.value * sm_mhz)}
     return out
+
+
+def debug_bounds(self_test=False):
+    """pic_debug_bounds: index violations counted by the check build (-1: production build)."""
+    v = C.c_int64(0)
+    rc = load().pic_debug_bounds(C.byref(v), C.c_int(1 if self_test else 0))
+    if rc != 0:
+        raise PicError(rc, "pic_debug_bounds")
+    return v.value
 
 
 def version():

@@ -28,6 +28,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "pic_check.cuh"
+
 namespace picb200 {
 
 #ifndef PIC_BLOCK
@@ -217,7 +219,9 @@ struct StartAcc {
 // O3: constants of cell c.  sA carries a one-face halo on both sides: sA[f+1] = A_f,
 // sA[0] = A_{n-1}, sA[n+1] = A_0, so the two faces of cell c are sA[c+1], sA[c+2].
 template <typename T>
-__device__ __forceinline__ void load_cell(const T* __restrict__ sA, T c_cap, Lane<T>& p, int32_t c) {
+__device__ __forceinline__ void load_cell(const T* __restrict__ sA, T c_cap, Lane<T>& p, int32_t c,
+                                          int32_t n_cells) {
+  c = chk(c, n_cells);
   const T AL = sA[c + 1], AR = sA[c + 2];
   p.AL = AL;
   p.dA = AR - AL;
@@ -232,6 +236,7 @@ __device__ __forceinline__ void deposit_visit(double* __restrict__ sF, int32_t n
   const T delta = xout - xin;
   const T right = delta * (T(0.5) * (xin + xout));
   const T left = delta - right;
+  c = chk(c, n_cells);
   const int32_t cr = (c + 1 == n_cells) ? 0 : c + 1;
   atomicAdd(&sF[c], (double)left);
   atomicAdd(&sF[cr], (double)right);
@@ -239,6 +244,7 @@ __device__ __forceinline__ void deposit_visit(double* __restrict__ sF, int32_t n
 
 __device__ __forceinline__ void flush_start(double* __restrict__ sF, int32_t n, StartAcc& s) {
   if (s.cell >= 0) {
+    s.cell = chk(s.cell, n);
     atomicAdd(&sF[s.cell], s.f0);
     atomicAdd(&sF[(s.cell + 1 == n) ? 0 : s.cell + 1], s.f1);
   }
@@ -292,9 +298,9 @@ __device__ __forceinline__ void deposit_endpoint(double* __restrict__ sF, int32_
   }
   if (len > 0) {
     const int32_t e = a + len;
-    atomicAdd(&sD[a], sgn);
-    if (e < n) atomicAdd(&sD[e], -sgn);
-    else if (e > n) { atomicAdd(&sD[0], sgn); atomicAdd(&sD[e - n], -sgn); }
+    atomicAdd(&sD[chk(a, n)], sgn);
+    if (e < n) atomicAdd(&sD[chk(e, n)], -sgn);
+    else if (e > n) { atomicAdd(&sD[0], sgn); atomicAdd(&sD[chk(e - n, n)], -sgn); }
   }
 }
 
@@ -321,6 +327,7 @@ __device__ __forceinline__ void warp_deposit_end(double* __restrict__ sF, int32_
       b += __shfl_xor_sync(kFull, b, o);
     }
     if (lane == leader) {
+      (void)chk(key, n);
       atomicAdd(&sF[key], a);
       atomicAdd(&sF[(key + 1 == n) ? 0 : key + 1], b);
     }
@@ -328,6 +335,7 @@ __device__ __forceinline__ void warp_deposit_end(double* __restrict__ sF, int32_
   }
   // ... lanes that end anywhere else (long, scattered orbits) add their own terms
   if (mine_left) {
+    (void)chk(et.cell, n);
     atomicAdd(&sF[et.cell], et.e0);
     atomicAdd(&sF[(et.cell + 1 == n) ? 0 : et.cell + 1], et.e1);
   }
@@ -468,7 +476,7 @@ __device__ __forceinline__ void substep(const MoverArgs<T>& a, const T* __restri
     p.u = uc;
     p.r -= dtc;
     if (EXACT_T) p.el += dtc;
-    load_cell<T>(sA, a.c_cap, p, cw);
+    load_cell<T>(sA, a.c_cap, p, cw, a.n_cells);
   }
 }
 
@@ -561,6 +569,7 @@ mover_kernel(const MoverArgs<T> a) {
             else if (a.deposit)
               deposit_endpoint(sF, sD, a.n_cells, acc, et, p.c0, (double)p.xa, c1, (double)p.xi, k);
             p.c = c1;
+            p.idx = chk(p.idx, a.n);
             if (a.xi1) {
               a.xi1[p.idx] = p.xi;
               a.v1[p.idx] = p.u * a.dx;
@@ -577,7 +586,7 @@ mover_kernel(const MoverArgs<T> a) {
           // ---- a1: ... and load the next particle of the range, if any.
           const uint32_t rank = (uint32_t)__popc(parked & lt_mask);
           if (rank < end - next) {
-            const uint32_t cand = next + rank;
+            const uint32_t cand = chk(next + rank, a.n);
             p.idx = cand;
             p.have = 1;
             p.xi = a.xi0[cand];
@@ -588,7 +597,7 @@ mover_kernel(const MoverArgs<T> a) {
             p.xa = p.xi;
             p.c0 = p.c;
             p.ns = 0; p.nc = 0; p.nr = 0;
-            load_cell<T>(sA, a.c_cap, p, p.c);
+            load_cell<T>(sA, a.c_cap, p, p.c, a.n_cells);
           }
         }
         if (!PER_VISIT) warp_deposit_end(sF, a.n_cells, lane, et);

@@ -91,7 +91,7 @@ __device__ __forceinline__ void cross2(const MoverArgs<float>& a, const float4* 
   put<S>(nu, uc);
   put<S>(used, dtc);
   float nAL, ndA, ncap;
-  load_cell3(sC + (p.c[S] & a.wrap_mask), nAL, ndA, ncap);
+  load_cell3(sC + chk(p.c[S] & a.wrap_mask, a.n_cells), nAL, ndA, ncap);
   put<S>(p.AL, nAL);
   put<S>(p.dA, ndA);
   put<S>(p.cap, ncap);
@@ -158,6 +158,7 @@ __device__ __forceinline__ void refill_slot(const MoverArgs<float>& a, double* _
     const float xi = get<S>(p.xi);
     if (a.deposit)
       deposit_endpoint(sF, sD, a.n_cells, acc, et, p.c0[S], (double)p.xa[S], c1, (double)xi, k);
+    p.idx[S] = chk(p.idx[S], a.n);
     if (a.xi1) {
       a.xi1[p.idx[S]] = xi;
       a.v1[p.idx[S]] = get<S>(p.u) * a.dx;
@@ -170,11 +171,11 @@ __device__ __forceinline__ void refill_slot(const MoverArgs<float>& a, double* _
     p.ns[S] = 0;
   }
   if (rank < end - next) {
-    const uint32_t cand = next + rank;
+    const uint32_t cand = chk(next + rank, a.n);
     p.idx[S] = cand;
     p.have[S] = 1;
     const float xi = a.xi0[cand];
-    const int32_t c = a.cell0[cand];
+    const int32_t c = chk(a.cell0[cand], a.n_cells);
     put<S>(p.xi, xi);
     put<S>(p.u, a.v0[cand] * a.inv_dx);
     put<S>(p.r, a.dt);

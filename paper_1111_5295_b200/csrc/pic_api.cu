@@ -12,6 +12,13 @@
 
 namespace picb200 {
 
+#if PIC_BOUNDS_CHECK
+__device__ unsigned long long g_bounds_violations = 0;   // pic_check.cuh
+namespace {
+__global__ void bounds_self_test_kernel(int* sink) { sink[chk(5, 3)] = 1; }   // one violation
+}  // namespace
+#endif
+
 int set_err(pic_handle* h, int code, const char* what, cudaError_t ce) {
   if (h) {
     h->err = what ? what : "";
@@ -59,7 +66,7 @@ int from_device(pic_handle* h, const double* dsrc, double* dst) {
 }
 
 VKey key_of(const pic_handle* h, const SpeciesState& S) {
-  return VKey{S.nx, S.nv, S.vmean, S.vinv, S.strided ? h->grid.n_cells : 0, 0};
+  return VKey{S.nx, S.nv, S.vmean, S.vinv, h->grid.n_cells, S.strided ? 1 : 0};
 }
 
 // exclusive scan of d_hist[0..nk) (three small kernels)
@@ -434,6 +441,30 @@ int pic_copy_state(pic_handle* dst, pic_handle* src) {
   }
   PIC_CUDA(dst, cudaGetLastError());
   dst->have_np1 = false;
+  return PIC_OK;
+}
+
+int pic_debug_bounds(int64_t* violations, int self_test) {
+  if (!violations) return PIC_ERR_ARG;
+#if PIC_BOUNDS_CHECK
+  if (self_test) {
+    int* d = nullptr;
+    if (cudaMalloc(&d, 3 * sizeof(int)) != cudaSuccess) { cudaGetLastError(); return PIC_ERR_CUDA; }
+    bounds_self_test_kernel<<<1, 1>>>(d);
+    cudaDeviceSynchronize();
+    cudaFree(d);
+  }
+  unsigned long long v = 0;
+  if (cudaDeviceSynchronize() != cudaSuccess ||
+      cudaMemcpyFromSymbol(&v, g_bounds_violations, sizeof v) != cudaSuccess) {
+    cudaGetLastError();
+    return PIC_ERR_CUDA;
+  }
+  *violations = (int64_t)v;
+#else
+  (void)self_test;
+  *violations = -1;   // not the check build
+#endif
   return PIC_OK;
 }
 

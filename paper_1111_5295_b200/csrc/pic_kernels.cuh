@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "pic_check.cuh"
+
 namespace picb200 {
 
 // Sort key of the binning: cell only (nx = nv = 1), or with PIC_FLAG_VSORT the phase-space cell
@@ -22,16 +24,17 @@ namespace picb200 {
 struct VKey {
   int32_t nx, nv;
   double vmean, vinv;   // vinv = nv / (8 sigma)
-  int32_t n_cells;      // > 0: strided order (v class, offset class, cell); 0: cell-major order
-  int32_t pad_;
+  int32_t n_cells;      // number of cells
+  int32_t strided;      // != 0: strided order (v class, offset class, cell); 0: cell-major order
 };
 __device__ __forceinline__ int32_t sort_key(const VKey& k, int32_t cell, double xi, double v) {
+  cell = chk(cell, k.n_cells);
   if (k.nv <= 1 && k.nx <= 1) return cell;
   const double t = (v - k.vmean) * k.vinv + 0.5 * k.nv;
   const int32_t b = (int32_t)fmin(fmax(t, 0.0), (double)(k.nv - 1));
   const int32_t xb = min((int32_t)(xi * k.nx), k.nx - 1);
-  if (k.n_cells > 0) return (b * k.nx + xb) * k.n_cells + cell;
-  return (cell * k.nx + xb) * k.nv + b;
+  const int32_t key = k.strided ? (b * k.nx + xb) * k.n_cells + cell : (cell * k.nx + xb) * k.nv + b;
+  return chk(key, (long long)k.n_cells * k.nx * k.nv);
 }
 
 // sum v, sum v^2 (fp64) -> out[0], out[1]
@@ -188,7 +191,8 @@ __global__ void scatter_kernel(long long n, const int32_t* __restrict__ cell_in,
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x) {
     const int32_t c = cell_in[i];
-    const int32_t dst = atomicAdd(&cursor[sort_key(vk, c, (double)xi_in[i], (double)v_in[i])], 1);
+    const int32_t dst =
+        chk(atomicAdd(&cursor[sort_key(vk, c, (double)xi_in[i], (double)v_in[i])], 1), n);
     cell_out[dst] = c;
     xi_out[dst] = xi_in[i];
     v_out[dst] = v_in[i];
@@ -249,7 +253,7 @@ __global__ void unpermute_kernel(long long n, const uint32_t* __restrict__ id,
                                  double* v_out, int32_t* cell_out, double* xi_out) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x) {
-    const uint32_t j = id[i];
+    const uint32_t j = chk(id[i], n);
     const double o = (double)xi[i];
     const int32_t c = cell[i];
     if (x_out) x_out[j] = ((double)c + o) * dx;
@@ -264,7 +268,7 @@ static __global__ void unpermute_counts_kernel(long long n, const uint32_t* __re
                                         uint32_t* a_out, uint32_t* b_out) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x) {
-    const uint32_t j = id[i];
+    const uint32_t j = chk(id[i], n);
     if (a_out) a_out[j] = a[i];
     if (b_out) b_out[j] = b[i];
   }
@@ -308,6 +312,7 @@ __global__ void sumsq_kernel(long long n, const T* __restrict__ v, double* __res
 constexpr int kRhoChunk = 32;
 __device__ __forceinline__ void rho_flush(double* __restrict__ rho, int32_t n_cells, int32_t c,
                                           double wl, double wc, double wr) {
+  c = chk(c, n_cells);
   atomicAdd(&rho[c == 0 ? n_cells - 1 : c - 1], wl);
   atomicAdd(&rho[c], wc);
   atomicAdd(&rho[c + 1 == n_cells ? 0 : c + 1], wr);
