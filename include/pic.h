@@ -35,7 +35,7 @@ typedef enum pic_status {
   PIC_ERR_PARTICLE = -3,   /* pic_init: a particle has non-finite x or v, or x outside [0,L) */
   PIC_ERR_SUBSTEP_CAP = -4,/* a particle hit max_substeps (A-9); results are still written   */
   PIC_ERR_STATE = -5,      /* call order: pic_residual before pic_set_step, commit before move */
-  PIC_ERR_UNSUPPORTED = -6 /* n_cells too large for the shared-memory grid of this build     */
+  PIC_ERR_UNSUPPORTED = -6 /* per-visit deposit asked for on a grid too large for shared memory */
 } pic_status;
 
 enum { PIC_FP32 = 0, PIC_FP64 = 1 };   /* arithmetic of the mover kernel (north_star (b))    */

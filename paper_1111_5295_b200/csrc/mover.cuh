@@ -69,6 +69,8 @@ struct MoverArgs {
   T dt, tol;
   double dt_exact;             // dt in fp64 (EXACT_T: the checkpointed remaining time starts here)
   double scale;                // w_q / dt : cell-unit deposit -> jbar contribution
+  unsigned char* grid_scratch; // GGRID: [gridDim.x][grid_stride] bytes of global memory that stand in
+  size_t grid_stride;          //        for the block's shared-memory grid (large n_cells)
   double* partial;             // [gridDim.x][n_cells] per-block sums (scaled)
   unsigned long long* queue;   // global index-range counter (zeroed before launch)
   unsigned long long* stats;   // [ST_COUNT] totals (accumulated)
@@ -494,10 +496,16 @@ template <> struct LaunchCfg<float> {
   static constexpr int block = kBlock;
 };
 
-template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2, bool EXACT_T = false>
+// GGRID: the per-block copy of the grid (field faces, fp64 sums, difference array) lives in
+// global memory instead of shared memory -- the fallback for grids whose n_cells (8 + 4 +
+// sizeof(T)) bytes exceed the 227 KB a block can have (S7 hard part 6).  The field is read
+// through L1/L2 and the deposits are global atomics on the block's own (L2-resident) row.
+template <typename T, bool CN_DIRECT, bool DIAG, bool PER_VISIT, bool POW2, bool EXACT_T = false,
+          bool GGRID = false>
 __global__ void __launch_bounds__(LaunchCfg<T>::block, LaunchCfg<T>::min_blocks)
 mover_kernel(const MoverArgs<T> a) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(16) unsigned char smem_dyn[];
+  unsigned char* smem_raw = GGRID ? a.grid_scratch + (size_t)blockIdx.x * a.grid_stride : smem_dyn;
   double* sF = reinterpret_cast<double*>(smem_raw);                 // [n] fp64 accumulators
   T* sA = reinterpret_cast<T*>(sF + a.n_cells);                     // [n+2] A on faces + halo
   int32_t* sD = reinterpret_cast<int32_t*>(sA + a.n_cells + 2);     // [n] difference array

@@ -199,14 +199,23 @@ int pic_rho(pic_handle* h, int which, double* rho_out) {
   const double dx = h->grid.length / ng;
   const int b = which == PIC_STATE_N ? h->cur : 1 - h->cur;
   PIC_CUDA(h, cudaMemsetAsync(h->d_resid, 0, sizeof(double) * ng, h->stream));
-  const size_t rho_smem = sizeof(double) * (size_t)ng;
+  size_t rho_smem = sizeof(double) * (size_t)ng;
+  const bool rho_global = rho_smem > 200 * 1024;   // large grid: no shared-memory copy of rho
+  if (rho_global) rho_smem = 0;
   if (rho_smem > 48 * 1024) {
     PIC_CUDA(h, cudaFuncSetAttribute(rho_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rho_smem));
     PIC_CUDA(h, cudaFuncSetAttribute(rho_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rho_smem));
   }
   for (auto& S : h->sp) {
     if (S.n == 0) continue;
-    if (h->elem == 4)
+    if (rho_global) {
+      if (h->elem == 4)
+        rho_kernel<float, false><<<rho_grid(h, S.n), 512, 0, h->stream>>>(
+            S.n, (const float*)S.xi[b], S.cell[b], ng, S.w_q / dx, h->d_resid);
+      else
+        rho_kernel<double, false><<<rho_grid(h, S.n), 512, 0, h->stream>>>(
+            S.n, (const double*)S.xi[b], S.cell[b], ng, S.w_q / dx, h->d_resid);
+    } else if (h->elem == 4)
       rho_kernel<float><<<rho_grid(h, S.n), 512, rho_smem, h->stream>>>(S.n, (const float*)S.xi[b], S.cell[b],
                                                               ng, S.w_q / dx, h->d_resid);
     else
@@ -233,7 +242,7 @@ int pic_destroy(pic_handle* h) {
   }
   cudaFree(h->dE_n); cudaFree(h->dE_step); cudaFree(h->dE_np1); cudaFree(h->d_jbar);
   cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue); cudaFree(h->d_stats);
-  cudaFree(h->d_hist); cudaFree(h->d_flag); cudaFree(h->d_scan);
+  cudaFree(h->d_hist); cudaFree(h->d_flag); cudaFree(h->d_scan); cudaFree(h->d_grid_scratch);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
   delete h;

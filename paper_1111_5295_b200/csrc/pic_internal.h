@@ -52,6 +52,9 @@ struct pic_handle {
   double* dE_np1 = nullptr;
   double* d_jbar = nullptr;
   double* d_resid = nullptr;
+  unsigned char* d_grid_scratch = nullptr;  // large grids: per-block grid copies in global memory
+  size_t grid_stride = 0;
+  int ggrid_max_blocks = 0;
   double* d_partial = nullptr; // [total_rows][n_cells]
   int total_rows = 0;
   unsigned long long* d_queue = nullptr;  // [n_species]

@@ -319,12 +319,16 @@ __device__ __forceinline__ void rho_flush(double* __restrict__ rho, int32_t n_ce
 }
 // Persistent blocks: each owns one contiguous span of the particle list and a shared-memory copy
 // of rho (dynamic, n_cells doubles), flushed to global memory once at the end.
-template <typename T>
+// SMEM = false (grids too large for shared memory): the sums go straight to global memory.
+template <typename T, bool SMEM = true>
 __global__ void rho_kernel(long long n, const T* __restrict__ xi, const int32_t* __restrict__ cell,
                            int32_t n_cells, double w_over_dx, double* __restrict__ rho) {
-  extern __shared__ double s_rho[];
-  for (int f = threadIdx.x; f < n_cells; f += blockDim.x) s_rho[f] = 0.0;
-  __syncthreads();
+  extern __shared__ double s_rho_dyn[];
+  double* s_rho = SMEM ? s_rho_dyn : rho;
+  if (SMEM) {
+    for (int f = threadIdx.x; f < n_cells; f += blockDim.x) s_rho[f] = 0.0;
+    __syncthreads();
+  }
   const long long stride = (long long)blockDim.x * kRhoChunk;
   const long long per_block = ((n + gridDim.x - 1) / gridDim.x + stride - 1) / stride * stride;
   const long long b0 = blockIdx.x * per_block;
@@ -361,9 +365,11 @@ __global__ void rho_kernel(long long n, const T* __restrict__ xi, const int32_t*
       rho_flush(s_rho, n_cells, cur, wl, wc, wr);
     }
   }
-  __syncthreads();
-  for (int f = threadIdx.x; f < n_cells; f += blockDim.x)
-    if (s_rho[f] != 0.0) atomicAdd(&rho[f], s_rho[f]);
+  if (SMEM) {
+    __syncthreads();
+    for (int f = threadIdx.x; f < n_cells; f += blockDim.x)
+      if (s_rho[f] != 0.0) atomicAdd(&rho[f], s_rho[f]);
+  }
 }
 
 // Histogram of per-particle counts (BJ configs[3]: sub-step histogram): bin k holds the particles

@@ -45,6 +45,18 @@ bool exact_time(const pic_params& P, double dt) {
   return (P.flags & PIC_FLAG_EXACT_TIME) != 0;
 }
 
+// GGRID instantiations (large grids): end-point deposit, generic wrap, plain time accounting.
+template <typename T, typename F>
+auto with_ggrid_kernel(bool direct, bool diag, F&& f) {
+  const int key = (direct ? 2 : 0) | (diag ? 1 : 0);
+  switch (key) {
+    case 0: return f(mover_kernel<T, false, false, false, false, false, true>);
+    case 1: return f(mover_kernel<T, false, true, false, false, false, true>);
+    case 2: return f(mover_kernel<T, true, false, false, false, false, true>);
+    default: return f(mover_kernel<T, true, true, false, false, false, true>);
+  }
+}
+
 template <typename T>
 cudaError_t set_smem_all(size_t bytes) {
   cudaError_t e = cudaSuccess;
@@ -102,6 +114,8 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
   const double tol_floor = 4.0 * (sizeof(T) == 4 ? 1.1920929e-7 : 2.220446049250313e-16);
   a.tol = (T)std::max(tol, tol_floor);
   a.scale = S.w_q / dt;
+  a.grid_scratch = h->d_grid_scratch;
+  a.grid_stride = h->grid_stride;
   a.partial = h->d_partial + (size_t)row0 * h->grid.n_cells;
   a.queue = h->d_queue + s;
   a.stats = h->d_stats;
@@ -125,6 +139,16 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
   S.last_blocks = S.grid_blocks;
   h->last_kernel = "mover_kernel";
   dim3 g(S.grid_blocks), b(LaunchCfg<T>::block);
+  if (h->d_grid_scratch) {
+    // large grid: the block's grid copy is a row of global memory (per-visit deposit and exact
+    // time accounting are not instantiated for it: end-point deposit, plain accounting)
+    h->last_kernel = "mover_kernel (global-memory grid)";
+    with_ggrid_kernel<T>(direct, diag, [&](auto k) {
+      k<<<g, b, 0, h->stream>>>(a);
+      return cudaSuccess;
+    });
+    return;
+  }
   with_kernel<T>(direct, diag, per_visit, a.wrap_mask != 0, exact, [&](auto k) {
     k<<<g, b, h->smem_bytes, h->stream>>>(a);
     return cudaSuccess;
@@ -139,18 +163,29 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
 int mover_configure(pic_handle* h) {
   const size_t bytes = h->elem == 4 ? mover_smem_bytes<float>(h->grid.n_cells)
                                     : mover_smem_bytes<double>(h->grid.n_cells);
-  if (bytes > 220 * 1024) return set_err(h, PIC_ERR_UNSUPPORTED, "n_cells too large for smem grid");
-  h->smem_bytes = bytes;
-  cudaError_t e = h->elem == 4 ? set_smem_all<float>(bytes) : set_smem_all<double>(bytes);
-  if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "cudaFuncSetAttribute(smem)", e);
-  int occ = h->elem == 4 ? occupancy<float>(bytes) : occupancy<double>(bytes);
-  if (occ < 1) return set_err(h, PIC_ERR_CUDA, "mover kernel does not fit on an SM");
+  const bool ggrid = bytes > 220 * 1024;       // the grid does not fit a block's shared memory
+  h->smem_bytes = ggrid ? 0 : bytes;
+  int occ;
+  if (ggrid) {
+    if (h->params.flags & PIC_FLAG_DEPOSIT_PER_VISIT)
+      return set_err(h, PIC_ERR_UNSUPPORTED, "per-visit deposit needs the grid in shared memory (n_cells too large)");
+    h->grid_stride = (bytes + 255) & ~(size_t)255;
+    // one wave of blocks, but no more rows of scratch than ~2 GB
+    const size_t budget = (size_t)2 << 30;
+    occ = (int)std::max<size_t>(1, std::min<size_t>(2, budget / h->grid_stride / h->sm_count));
+    h->ggrid_max_blocks = (int)std::max<size_t>(1, std::min<size_t>((size_t)h->sm_count * occ, budget / h->grid_stride));
+  } else {
+    cudaError_t e = h->elem == 4 ? set_smem_all<float>(bytes) : set_smem_all<double>(bytes);
+    if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "cudaFuncSetAttribute(smem)", e);
+    occ = h->elem == 4 ? occupancy<float>(bytes) : occupancy<double>(bytes);
+    if (occ < 1) return set_err(h, PIC_ERR_CUDA, "mover kernel does not fit on an SM");
+  }
   h->blocks_per_sm = occ;
   int rows = 0;
   for (auto& S : h->sp) {
     // persistent grid: one wave of resident blocks (a multiple of the SM count), fewer for
     // small problems so that every warp still gets a few refills' worth of particles.
-    const long long full = (long long)h->sm_count * occ;
+    const long long full = ggrid ? h->ggrid_max_blocks : (long long)h->sm_count * occ;
     const int block = h->elem == 4 ? LaunchCfg<float>::block : LaunchCfg<double>::block;
     const long long want = (S.n + block * 4 - 1) / (block * 4);
     S.grid_blocks = (int)std::max<long long>(1, std::min(full, want));
@@ -187,6 +222,12 @@ int mover_configure(pic_handle* h) {
     }
   }
   h->total_rows = rows;
+  if (ggrid) {
+    int maxb = 1;
+    for (auto& S : h->sp) maxb = std::max(maxb, S.grid_blocks);
+    cudaError_t e = cudaMalloc(&h->d_grid_scratch, h->grid_stride * (size_t)maxb);
+    if (e != cudaSuccess) return set_err(h, PIC_ERR_CUDA, "cudaMalloc(global-memory grid)", e);
+  }
   return PIC_OK;
 }
 

@@ -28,11 +28,11 @@ def ring(n_cells, n=10_007, vth=1.5, dt=4.0, seed=31):
                 species=[dict(name="e", q_over_m=-1.0, w_q=-length / n, x=x, v=v)])
 
 
-def tour(cfg, **kw):
+def tour(cfg, big=False, **kw):
     n_moves = 0
     for precision in ("fp32", "fp64"):
         for cn in ("direct", "picard"):
-            for flags in (0, B.PIC_FLAG_VSORT, B.PIC_FLAG_VSORT | B.PIC_FLAG_STRIDED,
+            for flags in (0, B.PIC_FLAG_VSORT, B.PIC_FLAG_COUNTS | B.PIC_FLAG_DIAG) if big else (0, B.PIC_FLAG_VSORT, B.PIC_FLAG_VSORT | B.PIC_FLAG_STRIDED,
                           B.PIC_FLAG_DEPOSIT_PER_VISIT, B.PIC_FLAG_COUNTS | B.PIC_FLAG_DIAG,
                           B.PIC_FLAG_VSORT | B.PIC_FLAG_ONE_PER_LANE, B.PIC_FLAG_EXACT_TIME):
                 pic = B.Pic(cfg["n_cells"], cfg["length"], cfg["species"], precision=precision,
@@ -68,6 +68,7 @@ def main():
     for ng in (1, 2, 3, 4, 48, 100):
         moves += tour(ring(ng))
     moves += tour(ring(8, n=257, vth=6.0, dt=3.0, seed=5))         # ~10 turns of the ring
+    moves += tour(ring(20_001, n=30_011), big=True)                # global-memory grid fallback
     moves += tour(kappa_cap_cfg(n=1500), **LOOSE)
     for kind in ("land", "turn"):
         moves += tour(landing_cfg(kind, dt=0.7, seed=1)[0], eps_a=1.0, eps_r=1.0)

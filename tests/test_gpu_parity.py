@@ -242,6 +242,39 @@ def test_non_power_of_two_grid(G, oracle, precision, n_cells):
         m["gpu"]["pic"].close()
 
 
+# ---- grids too large for a block's shared memory: the global-memory grid fallback (S7 hard part 6)
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("n_cells", [20_000, 100_003])
+def test_large_grid_global_memory_fallback(G, oracle, precision, n_cells):
+    from paper_1111_5295_b200 import binding as B
+    length = 0.7 * n_cells
+    xf = W.face_positions(n_cells, length)
+    n = 60_013
+    x = W.uniform01(41, 1, n) * length * (1 - 1e-12)
+    v = 1.5 * W.normal01(41, 2, n)
+    k = 2 * math.pi * round(n_cells / 150) / length            # ~150 cells per wavelength
+    cfg = dict(n_cells=n_cells, length=length, dt=4.0, tol=1e-12, E_n=0.2 * np.sin(k * xf),
+               E_np1=0.2 * np.sin(k * xf + 0.4),
+               species=[dict(name="e", q_over_m=-1.0, w_q=-length / n, x=x, v=v)])
+    for extra in (0, B.PIC_FLAG_VSORT):
+        m = G.parity(oracle, cfg, precision, extra_flags=extra, fast=True)
+        _report(f"n_cells={n_cells} {precision} flags+{extra} [{m['gpu']['kernel']}]", m)
+        assert m["gpu"]["kernel"] == "mover_kernel (global-memory grid)"
+        G.assert_parity(m, precision, max_flip_frac=2e-3)
+        pic = m["gpu"]["pic"]
+        # the diagnostics and the commit work on such grids too
+        dx = length / n_cells
+        end = pic.get_particles(0, B.PIC_STATE_NP1)
+        ref = oracle.rho(n_cells, length, cfg["species"][0]["w_q"], end["cell"], end["xi"] * dx)
+        assert G.rel_l2(pic.rho(B.PIC_STATE_NP1), ref) < 1e-12
+        pic.commit()
+        after = pic.get_particles(0, B.PIC_STATE_N)
+        assert np.array_equal(end["x"], after["x"]) and np.array_equal(end["v"], after["v"])
+        pic.close()
+    with pytest.raises(B.PicError):      # the per-visit deposit needs the grid in shared memory
+        B.Pic(n_cells, length, cfg["species"], precision=precision, flags=B.PIC_FLAG_DEPOSIT_PER_VISIT)
+
+
 # ---- Vlasov-Poisson variant: orbits without the current deposit, rho at the end
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_vp_variant_no_deposit(G, oracle, precision):
