@@ -20,10 +20,11 @@
 // (rounding coincidences: particles that end a step exactly on a face), the A-3 Picard cap
 // (picard_max = 1 is the explicit midpoint rule) -- each checked against what the mathematics
 // still fixes there (1 - kappa >= 1/2, sum dtau = dt, closed-form end state, P-5, P-6, P-9).
-// Parity unpinned (self-consistency only; the paper is silent on the CHOICE, the code that
-// implements it is pinned as above): the value kappa_max = 0.5 (A-2), the exact form of the
-// Picard convergence test (A-3), the face convention (A-5), the sub-step cap (A-9), the
-// face/cell index convention.
+// Every function and every branch of this file has at least one such pin.  What no pin can
+// settle is where the PAPER is silent and a reading had to be chosen:
+// the value kappa_max = 0.5 (A-2), the form of the Picard convergence test (A-3), the face
+// convention (A-5), the sub-step cap (A-9), the face/cell index convention.  The code that
+// implements each reading is pinned as above; the choice itself is a reading, not a result.
 //
 // Conventions (SURVEY 8 "Common notation"): periodic [0,L), n_cells uniform cells,
 // dx = L/n_cells; face f at x_f = f*dx; cell c spans faces c and (c+1) mod n_cells.
