@@ -14,13 +14,19 @@
 // P-3 Eq. 11 == Picard fixed point, P-4 estimator bound, P-5 crossing invariants +
 // bisection, P-6 per-cell discrete continuity, P-7 endpoint formula, P-8 mean current,
 // P-9 energy identity, P-10 refinement to the harmonic oscillator / RK reference,
-// P-11 hand-stepped tiny cases, P-12 residual sum; oracle_bin against hand values and the
+// P-11 hand-stepped tiny cases, P-12 residual sum; the A-9 sub-step cap (prefix property of the
+// aborted orbit); oracle_bin against hand values and the
 // identity cell*dx + s = x; and pins on workloads that EXECUTE the guard branches: the A-2
 // kappa cap (binding on most sub-steps), the O7 discriminant and crossing-time clamps
 // (rounding coincidences: particles that end a step exactly on a face), the A-3 Picard cap
 // (picard_max = 1 is the explicit midpoint rule) -- each checked against what the mathematics
 // still fixes there (1 - kappa >= 1/2, sum dtau = dt, closed-form end state, P-5, P-6, P-9).
-// Every function and every branch of this file has at least one such pin.  What no pin can
+// Every function of this file is pinned and every branch is executed by a pin (gcov: 294 of 300
+// lines under tests/test_oracle_pins.py), except three defensive guards that no input can reach
+// (DESIGN.md section 2): `dtau_c = dtau` for a_m == 0 while moving away from the exit face, the
+// lower clamp `dtau_c = 0` (a negative or NaN crossing time), and `w = 0` beyond the support of
+// the quadratic spline in oracle_rho (|xi| <= 3/2 always holds for the three cells visited).
+// What no pin can
 // settle is where the PAPER is silent and a reading had to be chosen:
 // the value kappa_max = 0.5 (A-2), the form of the Picard convergence test (A-3), the face
 // convention (A-5), the sub-step cap (A-9), the face/cell index convention.  The code that

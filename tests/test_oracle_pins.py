@@ -512,3 +512,43 @@ def test_guard_picard_cap(oracle):
     e = [abs(recs[k] - recs[50]) for k in (1, 2, 3)]
     assert e[0] > 1e-6 and e[1] == pytest.approx(kappa * e[0], rel=1e-6)
     assert e[2] == pytest.approx(kappa * e[1], rel=1e-4)
+
+
+def test_guard_substep_cap(oracle):
+    """A-9: an orbit that has taken max_substeps sub-steps with time left is aborted and counted.
+    The aborted orbit is exactly the first max_substeps sub-steps of the uncapped one (prefix
+    property, from the trace), the count is the number of particles that needed more, and
+    continuity (P-6) still holds to rounding: the deposit matches the distance actually
+    travelled, whether or not dt was used up."""
+    cfg = _multi_mode_cfg(n=800, dt=6.0)
+    sp = cfg["species"][0]
+    free = oracle_run(oracle, cfg)
+    need = free["species"][0]["n_sub"]
+    cap = int(np.median(need))
+    assert need.min() < cap < need.max()
+    out = oracle_run(oracle, cfg, oracle.make_params(tol=cfg["tol"], max_substeps=cap))
+    r, st = out["species"][0], out["stats"]
+    assert st.n_substep_cap == int((need > cap).sum()) > 100
+    assert np.all(r["n_sub"] == np.minimum(need, cap))
+    # untouched by the cap where it does not bind
+    ok = need <= cap
+    f = free["species"][0]
+    assert np.array_equal(r["v"][ok], f["v"][ok]) and np.array_equal(r["s"][ok], f["s"][ok])
+    # prefix property on the aborted ones
+    for i in np.nonzero(~ok)[0][:40]:
+        recs, _ = oracle.trace_particle(cfg["n_cells"], cfg["length"], sp["q_over_m"], sp["w_q"],
+                                        r["cell0"][i], r["s0"][i], r["v0"][i], cfg["E_n"],
+                                        cfg["E_np1"], cfg["dt"], oracle.make_params(tol=cfg["tol"]))
+        q = recs[cap - 1]
+        assert sum(t.dtau for t in recs[:cap]) < cfg["dt"]
+        assert r["v"][i] == q.v1
+        n_cells = cfg["n_cells"]
+        dx = cfg["length"] / n_cells
+        if q.crossed:       # the record ends on the face; the state has entered the neighbour
+            assert r["cell"][i] == (q.cell + q.crossed) % n_cells
+            assert r["s"][i] == (0.0 if q.crossed > 0 else dx)
+        else:
+            assert r["cell"][i] == q.cell and r["s"][i] == q.s1
+    res, div = continuity_residual(oracle, cfg, [(r["cell0"], r["s0"])], [(r["cell"], r["s"])],
+                                   out["jbar"])
+    assert np.linalg.norm(res) < 1e-12 * np.linalg.norm(div)
