@@ -196,8 +196,9 @@ void free_all(pic_handle* h) {
     cudaFree(S.nsub); cudaFree(S.ncross);
   }
   cudaFree(h->dE_n); cudaFree(h->dE_step); cudaFree(h->dE_np1); cudaFree(h->d_jbar);
-  cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue); cudaFree(h->d_stats);
+  cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue);   // d_stats is part of d_queue
   cudaFree(h->d_hist); cudaFree(h->d_flag); cudaFree(h->d_scan); cudaFree(h->d_grid_scratch);
+  if (h->h_pin) cudaFreeHost(h->h_pin);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
 }
@@ -265,9 +266,11 @@ int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species,
   INIT_CUDA(cudaMalloc(&h->dE_step, sizeof(double) * ng));
   INIT_CUDA(cudaMalloc(&h->dE_np1, sizeof(double) * ng));
   INIT_CUDA(cudaMalloc(&h->d_jbar, sizeof(double) * ng));
-  INIT_CUDA(cudaMalloc(&h->d_resid, sizeof(double) * ng));
-  INIT_CUDA(cudaMalloc(&h->d_queue, sizeof(unsigned long long) * n_species));
-  INIT_CUDA(cudaMalloc(&h->d_stats, sizeof(unsigned long long) * ST_COUNT));
+  INIT_CUDA(cudaMalloc(&h->d_resid, sizeof(double) * (ng + 1)));   // + the sub-step-cap count
+  // queue counters and stats in one allocation: one memset per move
+  INIT_CUDA(cudaMalloc(&h->d_queue, sizeof(unsigned long long) * (n_species + ST_COUNT)));
+  h->d_stats = h->d_queue + n_species;
+  INIT_CUDA(cudaMallocHost(&h->h_pin, sizeof(double) * 2 * (ng + 1)));   // staging of E in / R out
 #ifndef PIC_KEYCAP_LOG2
 #define PIC_KEYCAP_LOG2 24
 #endif
@@ -333,17 +336,11 @@ int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species,
   return PIC_OK;
 }
 
-int pic_move_accumulate(pic_handle* h, const double* E_n, const double* E_np1, double dt,
-                        double tol, double* jbar_out) {
-  if (!h) return PIC_ERR_ARG;
-  if (!E_n || !E_np1 || !(dt > 0.0) || !(tol >= 0.0)) return set_err(h, PIC_ERR_ARG, "pic_move_accumulate: bad argument");
-  const double *dEn = nullptr, *dEp = nullptr;
+// a0-a8 for every species with the fields already on the device: launches only
+static int move_device(pic_handle* h, const double* dEn, const double* dEp, double dt, double tol) {
   int rc;
-  if ((rc = to_device(h, E_n, h->dE_n, &dEn)) != PIC_OK) return rc;
-  if ((rc = to_device(h, E_np1, h->dE_np1, &dEp)) != PIC_OK) return rc;
   const int ns = (int)h->sp.size();
-  PIC_CUDA(h, cudaMemsetAsync(h->d_queue, 0, sizeof(unsigned long long) * ns, h->stream));
-  PIC_CUDA(h, cudaMemsetAsync(h->d_stats, 0, sizeof(unsigned long long) * ST_COUNT, h->stream));
+  PIC_CUDA(h, cudaMemsetAsync(h->d_queue, 0, sizeof(unsigned long long) * (ns + ST_COUNT), h->stream));
   PIC_CUDA(h, cudaEventRecord(h->ev0, h->stream));
   int row = 0;
   for (int s = 0; s < ns; ++s) {
@@ -357,6 +354,18 @@ int pic_move_accumulate(pic_handle* h, const double* E_n, const double* E_np1, d
   h->launches++;
   PIC_CUDA(h, cudaGetLastError());
   h->have_np1 = !(h->params.flags & PIC_FLAG_NO_STORE);
+  return PIC_OK;
+}
+
+int pic_move_accumulate(pic_handle* h, const double* E_n, const double* E_np1, double dt,
+                        double tol, double* jbar_out) {
+  if (!h) return PIC_ERR_ARG;
+  if (!E_n || !E_np1 || !(dt > 0.0) || !(tol >= 0.0)) return set_err(h, PIC_ERR_ARG, "pic_move_accumulate: bad argument");
+  const double *dEn = nullptr, *dEp = nullptr;
+  int rc;
+  if ((rc = to_device(h, E_n, h->dE_n, &dEn)) != PIC_OK) return rc;
+  if ((rc = to_device(h, E_np1, h->dE_np1, &dEp)) != PIC_OK) return rc;
+  if ((rc = move_device(h, dEn, dEp, dt, tol)) != PIC_OK) return rc;
   const bool host_out = jbar_out && !is_device_ptr(jbar_out);
   unsigned long long capped = 0;
   if (host_out)   // rides on the synchronisation the host copy of jbar needs anyway
@@ -379,29 +388,47 @@ int pic_set_step(pic_handle* h, const double* E_n, double dt, double tol) {
   return PIC_OK;
 }
 
-int pic_residual(pic_handle* h, const double* E_np1, double* resid_out) {
+}  // extern "C"
+
+// pic_residual with the kind of each pointer known (1 = device, 0 = host, -1 = ask the driver):
+// the JFNK driver calls it 13-36 times per time step with host arrays, so the host side is kept
+// to one staged copy in, the launches, and one staged copy out that also carries the count of
+// orbits cut off at max_substeps (A-9).
+int picb200::residual_impl(pic_handle* h, const double* E_np1, double* resid_out, int e_dev, int r_dev) {
   if (!h) return PIC_ERR_ARG;
   if (!h->have_step) return set_err(h, PIC_ERR_STATE, "pic_residual before pic_set_step");
   if (!E_np1 || !resid_out) return set_err(h, PIC_ERR_ARG, "pic_residual: NULL argument");
-  const double* dEp = nullptr;
+  const int32_t ng = h->grid.n_cells;
+  if (e_dev < 0) e_dev = is_device_ptr(E_np1) ? 1 : 0;
+  if (r_dev < 0) r_dev = is_device_ptr(resid_out) ? 1 : 0;
+  const double* dEp = E_np1;
   int rc;
-  if ((rc = to_device(h, E_np1, h->dE_np1, &dEp)) != PIC_OK) return rc;
-  if ((rc = pic_move_accumulate(h, h->dE_step, dEp, h->step_dt, h->step_tol, nullptr)) != PIC_OK)
-    return rc;
-  residual_kernel<<<1, 256, 0, h->stream>>>(h->grid.n_cells, h->dE_step, dEp, h->step_dt,
-                                            h->d_jbar, h->d_resid);
+  if (!e_dev) {
+    std::memcpy(h->h_pin, E_np1, sizeof(double) * ng);
+    PIC_CUDA(h, cudaMemcpyAsync(h->dE_np1, h->h_pin, sizeof(double) * ng, cudaMemcpyHostToDevice, h->stream));
+    dEp = h->dE_np1;
+  }
+  if ((rc = move_device(h, h->dE_step, dEp, h->step_dt, h->step_tol)) != PIC_OK) return rc;
+  residual_kernel<<<1, 256, 0, h->stream>>>(ng, h->dE_step, dEp, h->step_dt, h->d_jbar, h->d_resid,
+                                            h->d_stats + ST_SUBSTEP_CAP);
   h->launches++;
   PIC_CUDA(h, cudaGetLastError());
-  // A-9: orbits cut off at max_substeps leave dt unused; report it with the residual (the count
-  // rides on the synchronisation the host copy needs anyway)
-  unsigned long long capped = 0;
-  const bool host_out = !is_device_ptr(resid_out);
-  if (host_out)
-    PIC_CUDA(h, cudaMemcpyAsync(&capped, h->d_stats + ST_SUBSTEP_CAP, sizeof capped,
-                                cudaMemcpyDeviceToHost, h->stream));
-  if ((rc = from_device(h, h->d_resid, resid_out)) != PIC_OK) return rc;
-  if (capped) return set_err(h, PIC_ERR_SUBSTEP_CAP, "particles cut off at max_substeps");
+  if (r_dev) {
+    PIC_CUDA(h, cudaMemcpyAsync(resid_out, h->d_resid, sizeof(double) * ng, cudaMemcpyDeviceToDevice, h->stream));
+    return PIC_OK;     // no synchronisation, so no cap report (pic_get_stats has the count)
+  }
+  double* out = h->h_pin + (ng + 1);
+  PIC_CUDA(h, cudaMemcpyAsync(out, h->d_resid, sizeof(double) * (ng + 1), cudaMemcpyDeviceToHost, h->stream));
+  PIC_CUDA(h, cudaStreamSynchronize(h->stream));
+  std::memcpy(resid_out, out, sizeof(double) * ng);
+  if (out[ng] != 0.0) return set_err(h, PIC_ERR_SUBSTEP_CAP, "particles cut off at max_substeps");
   return PIC_OK;
+}
+
+extern "C" {
+
+int pic_residual(pic_handle* h, const double* E_np1, double* resid_out) {
+  return picb200::residual_impl(h, E_np1, resid_out, -1, -1);
 }
 
 int pic_copy_state(pic_handle* dst, pic_handle* src) {

@@ -241,8 +241,9 @@ int pic_destroy(pic_handle* h) {
     cudaFree(S.nsub); cudaFree(S.ncross);
   }
   cudaFree(h->dE_n); cudaFree(h->dE_step); cudaFree(h->dE_np1); cudaFree(h->d_jbar);
-  cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue); cudaFree(h->d_stats);
+  cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue);   // d_stats is part of d_queue
   cudaFree(h->d_hist); cudaFree(h->d_flag); cudaFree(h->d_scan); cudaFree(h->d_grid_scratch);
+  if (h->h_pin) cudaFreeHost(h->h_pin);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
   delete h;

@@ -57,8 +57,9 @@ struct pic_handle {
   int ggrid_max_blocks = 0;
   double* d_partial = nullptr; // [total_rows][n_cells]
   int total_rows = 0;
-  unsigned long long* d_queue = nullptr;  // [n_species]
-  unsigned long long* d_stats = nullptr;  // [ST_COUNT]
+  unsigned long long* d_queue = nullptr;  // [n_species] + [ST_COUNT]: one allocation, one memset
+  unsigned long long* d_stats = nullptr;  // = d_queue + n_species
+  double* h_pin = nullptr;                // pinned host staging, 2 x (n_cells + 1)
   int32_t* d_hist = nullptr;              // [n_keys + 1] binning scratch
   long long n_keys = 0;
   int32_t* d_scan = nullptr;              // [n_keys / 4096 + 1] chunk sums of the scan
@@ -78,6 +79,8 @@ bool is_device_ptr(const void* p);
 int launch_mover(pic_handle* h, int s, const double* dE_n, const double* dE_np1, double dt,
                  double tol, int row0);
 int mover_configure(pic_handle* h);
+// pic_residual with known pointer kinds (1 device, 0 host, -1 unknown); pic_api.cu
+int residual_impl(pic_handle* h, const double* E_np1, double* resid_out, int e_dev, int r_dev);
 
 }  // namespace picb200
 

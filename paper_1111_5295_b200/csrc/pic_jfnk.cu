@@ -32,7 +32,7 @@ struct Jfnk {
     const uint32_t f0 = hh->params.flags;
     hh->params.flags = store ? (f0 & ~PIC_FLAG_NO_STORE) : (f0 | PIC_FLAG_NO_STORE);
     const bool keep = hh->have_np1;
-    const int rc = pic_residual(hh, E.data(), R.data());
+    const int rc = residual_impl(hh, E.data(), R.data(), 0, 0);   // host vectors
     if (!store) hh->have_np1 = keep;   // a Krylov call leaves the stored state n+1 untouched
     hh->params.flags = f0;
     return rc;

@@ -225,9 +225,12 @@ reduce_rows_kernel(int rows, int32_t n_cells, const double* __restrict__ partial
 }
 
 // a9: R_f = (E^{n+1}_f - E^n_f)/dt + jbar_f - <jbar>  (eps0 = 1).  One block.
+// resid[n_cells] receives the number of orbits cut off at max_substeps (A-9), so that one copy
+// brings both back.
 static __global__ void residual_kernel(int32_t n_cells, const double* __restrict__ E_n,
                                 const double* __restrict__ E_np1, double dt,
-                                const double* __restrict__ jbar, double* __restrict__ resid) {
+                                const double* __restrict__ jbar, double* __restrict__ resid,
+                                const unsigned long long* __restrict__ n_capped) {
   __shared__ double red[32];
   __shared__ double mean;
   double s = 0.0;
@@ -243,6 +246,7 @@ static __global__ void residual_kernel(int32_t n_cells, const double* __restrict
   __syncthreads();
   for (int f = threadIdx.x; f < n_cells; f += blockDim.x)
     resid[f] = (E_np1[f] - E_n[f]) / dt + jbar[f] - mean;
+  if (threadIdx.x == 0) resid[n_cells] = (double)*n_capped;
 }
 
 // Getter: un-permute to the original order.  Any output may be NULL.
