@@ -199,6 +199,8 @@ void free_all(pic_handle* h) {
   cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue);   // d_stats is part of d_queue
   cudaFree(h->d_hist); cudaFree(h->d_flag); cudaFree(h->d_scan); cudaFree(h->d_grid_scratch);
   if (h->h_pin) cudaFreeHost(h->h_pin);
+  for (auto& e : h->graphs) cudaGraphExecDestroy(e.exec);
+  if (h->own_stream) cudaStreamDestroy(h->own_stream);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
 }
@@ -337,17 +339,18 @@ int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species,
 }
 
 // a0-a8 for every species with the fields already on the device: launches only
-static int move_device(pic_handle* h, const double* dEn, const double* dEp, double dt, double tol) {
+static int move_device(pic_handle* h, const double* dEn, const double* dEp, double dt, double tol,
+                       bool timed = true) {
   int rc;
   const int ns = (int)h->sp.size();
   PIC_CUDA(h, cudaMemsetAsync(h->d_queue, 0, sizeof(unsigned long long) * (ns + ST_COUNT), h->stream));
-  PIC_CUDA(h, cudaEventRecord(h->ev0, h->stream));
+  if (timed) PIC_CUDA(h, cudaEventRecord(h->ev0, h->stream));
   int row = 0;
   for (int s = 0; s < ns; ++s) {
     if ((rc = launch_mover(h, s, dEn, dEp, dt, tol, row)) != PIC_OK) return rc;
     row += h->sp[s].last_blocks;
   }
-  PIC_CUDA(h, cudaEventRecord(h->ev1, h->stream));
+  if (timed) PIC_CUDA(h, cudaEventRecord(h->ev1, h->stream));
   const int32_t ng = h->grid.n_cells;
   reduce_rows_kernel<<<(ng + kRedCols - 1) / kRedCols, dim3(kRedCols, kRedRows), 0, h->stream>>>(
       row, ng, h->d_partial, h->d_jbar);
@@ -390,6 +393,71 @@ int pic_set_step(pic_handle* h, const double* E_n, double dt, double tol) {
 
 }  // extern "C"
 
+// One residual evaluation from host E^{n+1} to host R as a CUDA graph, captured once per
+// (flags, dt, tol) and replayed: at 1-4 M particles a pass is 0.1-0.2 ms of kernels, and the five
+// launches, two copies and two event records around them were a quarter of its wall time.
+// Returns PIC_ERR_UNSUPPORTED if the stream cannot be captured (the caller falls back).
+static int residual_graph(pic_handle* h, const double* E_np1, double* resid_out) {
+  const int32_t ng = h->grid.n_cells;
+  cudaStream_t st = h->stream;
+  if (!st) {   // the legacy default stream cannot be captured: a blocking stream of our own
+    if (!h->own_stream && cudaStreamCreate(&h->own_stream) != cudaSuccess) {
+      cudaGetLastError();
+      return PIC_ERR_UNSUPPORTED;
+    }
+    st = h->own_stream;
+  }
+  double* out = h->h_pin + (ng + 1);
+  pic_handle::ResidualGraph* g = nullptr;
+  for (auto& e : h->graphs)
+    if (e.flags == h->params.flags && e.dt == h->step_dt && e.tol == h->step_tol) g = &e;
+  if (!g) {
+    if (h->graphs.size() >= 8) {
+      for (auto& e : h->graphs) cudaGraphExecDestroy(e.exec);
+      h->graphs.clear();
+    }
+    cudaStream_t user = h->stream;
+    const long long l0 = h->launches;
+    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+      cudaGetLastError();
+      return PIC_ERR_UNSUPPORTED;
+    }
+    h->stream = st;
+    int rc = PIC_OK;
+    cudaError_t ce = cudaMemcpyAsync(h->dE_np1, h->h_pin, sizeof(double) * ng, cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) rc = move_device(h, h->dE_step, h->dE_np1, h->step_dt, h->step_tol, false);
+    if (ce == cudaSuccess && rc == PIC_OK) {
+      residual_kernel<<<1, 256, 0, st>>>(ng, h->dE_step, h->dE_np1, h->step_dt, h->d_jbar, h->d_resid,
+                                         h->d_stats + ST_SUBSTEP_CAP);
+      h->launches++;
+      ce = cudaMemcpyAsync(out, h->d_resid, sizeof(double) * (ng + 1), cudaMemcpyDeviceToHost, st);
+    }
+    h->stream = user;
+    cudaGraph_t graph = nullptr;
+    cudaError_t ee = cudaStreamEndCapture(st, &graph);
+    cudaGraphExec_t exec = nullptr;
+    if (ce == cudaSuccess && rc == PIC_OK && ee == cudaSuccess && graph)
+      ee = cudaGraphInstantiate(&exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    const long long nl = h->launches - l0;
+    h->launches = l0;
+    if (ce != cudaSuccess || rc != PIC_OK || ee != cudaSuccess || !exec) {
+      cudaGetLastError();
+      return PIC_ERR_UNSUPPORTED;
+    }
+    h->graphs.push_back({h->params.flags, h->step_dt, h->step_tol, exec, nl});
+    g = &h->graphs.back();
+  }
+  std::memcpy(h->h_pin, E_np1, sizeof(double) * ng);
+  PIC_CUDA(h, cudaGraphLaunch(g->exec, st));
+  h->launches += g->n_launches;
+  h->have_np1 = !(h->params.flags & PIC_FLAG_NO_STORE);
+  PIC_CUDA(h, cudaStreamSynchronize(st));
+  std::memcpy(resid_out, out, sizeof(double) * ng);
+  if (out[ng] != 0.0) return set_err(h, PIC_ERR_SUBSTEP_CAP, "particles cut off at max_substeps");
+  return PIC_OK;
+}
+
 // pic_residual with the kind of each pointer known (1 = device, 0 = host, -1 = ask the driver):
 // the JFNK driver calls it 13-36 times per time step with host arrays, so the host side is kept
 // to one staged copy in, the launches, and one staged copy out that also carries the count of
@@ -403,6 +471,13 @@ int picb200::residual_impl(pic_handle* h, const double* E_np1, double* resid_out
   if (r_dev < 0) r_dev = is_device_ptr(resid_out) ? 1 : 0;
   const double* dEp = E_np1;
   int rc;
+  if (!e_dev && !r_dev && !h->graphs_off) {
+    // host in, host out (the JFNK driver): the whole evaluation is one CUDA graph per
+    // (flags, dt, tol) -- copy in, memset, movers, row sum, residual, copy out
+    rc = residual_graph(h, E_np1, resid_out);
+    if (rc != PIC_ERR_UNSUPPORTED) return rc;
+    h->graphs_off = true;     // capture not possible here: plain launches
+  }
   if (!e_dev) {
     std::memcpy(h->h_pin, E_np1, sizeof(double) * ng);
     PIC_CUDA(h, cudaMemcpyAsync(h->dE_np1, h->h_pin, sizeof(double) * ng, cudaMemcpyHostToDevice, h->stream));

@@ -244,6 +244,8 @@ int pic_destroy(pic_handle* h) {
   cudaFree(h->d_resid); cudaFree(h->d_partial); cudaFree(h->d_queue);   // d_stats is part of d_queue
   cudaFree(h->d_hist); cudaFree(h->d_flag); cudaFree(h->d_scan); cudaFree(h->d_grid_scratch);
   if (h->h_pin) cudaFreeHost(h->h_pin);
+  for (auto& e : h->graphs) cudaGraphExecDestroy(e.exec);
+  if (h->own_stream) cudaStreamDestroy(h->own_stream);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
   delete h;

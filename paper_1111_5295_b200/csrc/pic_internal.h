@@ -65,6 +65,16 @@ struct pic_handle {
   int32_t* d_scan = nullptr;              // [n_keys / 4096 + 1] chunk sums of the scan
   int32_t* d_flag = nullptr;              // validation flag
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  // CUDA graphs of one residual evaluation with host vectors (pic_api.cu: residual_impl)
+  struct ResidualGraph {
+    uint32_t flags;
+    double dt, tol;
+    cudaGraphExec_t exec;
+    long long n_launches;
+  };
+  std::vector<ResidualGraph> graphs;
+  cudaStream_t own_stream = nullptr;   // for graph launches when `stream` is the legacy default stream
+  bool graphs_off = false;             // a capture failed once: plain launches from then on
   pic_stats stats{};
   long long launches = 0;
   const char* last_kernel = "";   // name of the mover kernel of the last launch
