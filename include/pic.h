@@ -102,7 +102,9 @@ typedef struct pic_stats { /* totals of the LAST pic_move_accumulate over all sp
   int64_t n_neg_disc;      /* crossings with v^2 + 2 a_m d clamped at 0       (DIAG)           */
   int64_t n_clamped_tau;   /* crossings whose dtau_c was clamped to [0,dtau]  (DIAG)           */
   int64_t n_launches;      /* kernels this library launched since pic_init                     */
-  double last_move_ms;     /* device time of the last mover kernel(s), CUDA events on stream   */
+  double last_move_ms;     /* device time of the mover kernel(s) of the last pic_move_accumulate
+                              (CUDA events on the stream; graph-replayed pic_residual calls with
+                              host arrays are not timed)                                       */
 } pic_stats;
 
 /* pic_init — "pic_init(grid, species, particles)" (north_star (a); S8(b)).
@@ -137,7 +139,11 @@ int pic_set_step(pic_handle* h, const double* E_n, double dt, double tol);
  *   R_f = eps0 (E^{n+1}_f - E^n_f)/dt + jbar_f - <jbar>,  <jbar> = mean over faces, eps0 = 1,
  * with jbar from pic_move_accumulate(E^n, E_np1, dt, tol).  resid_out[n_cells].
  * Returns PIC_ERR_SUBSTEP_CAP (the residual is still written) if any particle was cut off at
- * max_substeps; checked when resid_out is a HOST pointer, as for pic_move_accumulate. */
+ * max_substeps; checked when resid_out is a HOST pointer, as for pic_move_accumulate.
+ * With HOST E_np1 and HOST resid_out (the JFNK driver's case) the whole evaluation -- staged copy
+ * in, movers, row sum, residual, copy out -- is captured once per (flags, dt, tol) as a CUDA graph
+ * and replayed; if `stream` is the legacy default stream the replay runs on a blocking stream of
+ * the library's own, which orders with the default stream as usual. */
 int pic_residual(pic_handle* h, const double* E_np1, double* resid_out);
 
 /* pic_commit — accept state n+1 of the last pic_move_accumulate as the new state n and re-bin
