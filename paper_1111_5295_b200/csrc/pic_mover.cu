@@ -191,10 +191,21 @@ int mover_configure(pic_handle* h) {
     S.grid_blocks = (int)std::max<long long>(1, std::min(full, want));
     const long long warps = (long long)S.grid_blocks * (block / 32);
     long long tile = S.n / (warps * 8);                 // >= 8 claims per warp
+// Smallest index range a warp claims from the queue.  Every claim is a global atomic whose
+// latency the warp waits out, so small species (1-4 M particles: fewer than 500 per warp) run
+// faster with a few long claims per warp than with one claim per refill, even though some warps
+// then get no work: 128 (one particle per lane) / 256 (two) measured best on configs[1] and [4]
+// (mover pass 0.104 -> 0.068 ms, 0.189 -> 0.163 ms; profiles/r2_bench.md).
+#ifndef PIC_TILE_MIN
+#define PIC_TILE_MIN 128
+#endif
+#ifndef PIC_TILE_MIN2
+#define PIC_TILE_MIN2 256
+#endif
 #ifndef PIC_TILE_MAX
 #define PIC_TILE_MAX 512
 #endif
-    tile = std::max<long long>(32, std::min<long long>(PIC_TILE_MAX, tile / 32 * 32));
+    tile = std::max<long long>(PIC_TILE_MIN, std::min<long long>(PIC_TILE_MAX, tile / 32 * 32));
     S.tile = (int)tile;
     rows += S.grid_blocks;
   }
@@ -214,7 +225,7 @@ int mover_configure(pic_handle* h) {
         S.grid_blocks2 = (int)std::max<long long>(1, std::min<long long>(std::min(full, want), S.grid_blocks));
         const long long warps = (long long)S.grid_blocks2 * (kBlock2 / 32);
         long long tile = S.n / (warps * 8);
-        tile = std::max<long long>(64, std::min<long long>(PIC_TILE_MAX, tile / 64 * 64));
+        tile = std::max<long long>(PIC_TILE_MIN2, std::min<long long>(PIC_TILE_MAX, tile / 64 * 64));
         S.tile2 = (int)tile;
       }
     } else {
