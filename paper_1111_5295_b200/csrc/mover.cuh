@@ -343,6 +343,21 @@ __device__ __forceinline__ void warp_deposit_end(double* __restrict__ sF, int32_
   }
 }
 
+// Warp-uniform: the lanes flagged in `flush` hand their start-cell accumulators to the block
+// sums.  Lanes of a warp walk through the binned particle list together, so they leave a start
+// cell in the same refill: flushed one by one inside deposit_endpoint, 32 lanes hit the same two
+// addresses with the CAS loop of the shared fp64 add and spin ~30 rounds each (42 % of the
+// instructions of a 2 M ion pass, profiles/r2_bench.md); summed over the warp first it is one add
+// per face.
+__device__ __forceinline__ void warp_flush_start(double* __restrict__ sF, int32_t n, int lane,
+                                                 StartAcc& acc, bool flush) {
+  if (!__any_sync(kFull, flush)) return;
+  EndTerms t;
+  t.e0 = acc.f0; t.e1 = acc.f1; t.cell = flush ? acc.cell : 0; t.pending = flush;
+  warp_deposit_end(sF, n, lane, t);
+  if (flush) { acc.cell = -1; acc.f0 = acc.f1 = 0.0; }
+}
+
 // ---- a8: one flush per block.  Inclusive prefix sum of the difference array over the
 // faces (each thread owns a contiguous chunk), then scaled block sums -> this block's row of
 // `partial`.  Called by every thread of the block after its warps have left the particle loop.
@@ -567,6 +582,9 @@ mover_kernel(const MoverArgs<T> a) {
         }
         EndTerms et;
         et.pending = false; et.cell = 0; et.e0 = et.e1 = 0.0;
+        if (!PER_VISIT)
+          warp_flush_start(sF, a.n_cells, lane, acc,
+                           !(p.r > T(0)) && p.have && a.deposit && acc.cell >= 0 && p.c0 != acc.cell);
         if (!(p.r > T(0))) {
           // ---- a7: store the parked result (state n+1) and deposit its current ...
           if (p.have) {

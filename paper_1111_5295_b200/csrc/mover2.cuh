@@ -255,8 +255,14 @@ mover2_kernel(const MoverArgs<float> a) {
           }
         }
         EndTerms et0, et1;
+        // a lane's start-cell sums leave for the block sums when its next finished orbit began in
+        // another cell: all lanes of the warp do that in the same refill, so sum them first
+        warp_flush_start(sF, a.n_cells, lane, acc,
+                         !(p.r.x > 0.0f) && p.have[0] && a.deposit && acc.cell >= 0 && p.c0[0] != acc.cell);
         refill_slot<0>(a, sF, sD, sC, p, acc, et0, (uint32_t)__popc(pk0 & lt_mask), next, end,
                        tot_sub, capped);
+        warp_flush_start(sF, a.n_cells, lane, acc,
+                         !(p.r.y > 0.0f) && p.have[1] && a.deposit && acc.cell >= 0 && p.c0[1] != acc.cell);
         refill_slot<1>(a, sF, sD, sC, p, acc, et1, (uint32_t)(n0 + __popc(pk1 & lt_mask)), next, end,
                        tot_sub, capped);
         // the two slots of a lane mostly end in the same cell: add them up first, then one
