@@ -57,7 +57,9 @@ struct MoverArgs {
   int32_t n_cells;
   int32_t max_substeps;
   int32_t picard_max;
-  int32_t tile;                // particles per claimed index range (multiple of 32)
+  int32_t tile;                // particles per claimed index range (multiple of 32), at most
+  int32_t tile_min;            // ... and at least; in between: what is left / guide_div
+  uint32_t guide_div;          // guided self-scheduling: 0 = always `tile`
   int32_t refill_threshold;    // parked lanes needed before a refill
   int32_t wrap_mask;           // n_cells - 1 if n_cells is a power of two, else 0
   int32_t deposit;             // 0 = VP variant: orbits only, no current deposit
@@ -177,6 +179,18 @@ constexpr int kGroup = PIC_UNROLL;        // sub-steps between two "any lane sti
 constexpr int kInner = PIC_KINNER;        // sub-step rounds between two refill votes
 constexpr int kRefill = PIC_REFILL;       // parked lanes needed before a refill (cell binning)
 constexpr int kRefillVsort = PIC_REFILL_VSORT;  // same with (cell, velocity class) binning
+
+// Guided self-scheduling of the work queue: a warp claims `tile` particles while plenty are left
+// and shrinking ranges (what is left / guide_div, never below tile_min) towards the end, so that
+// the last ranges are short and the warps of the grid finish together.  `left` is the warp's own
+// view (from the end of its last range), an over-estimate.
+__device__ __forceinline__ uint32_t claim_size(int32_t tile, int32_t tile_min, uint32_t guide_div,
+                                               uint32_t left) {
+  if (guide_div == 0) return (uint32_t)tile;
+  uint32_t w = (left / guide_div) & ~63u;
+  w = w < (uint32_t)tile_min ? (uint32_t)tile_min : w;
+  return w > (uint32_t)tile ? (uint32_t)tile : w;
+}
 
 // Per-lane particle registers.  r > 0 <=> an orbit is in flight.
 template <typename T>
@@ -571,13 +585,14 @@ mover_kernel(const MoverArgs<T> a) {
       if (go) {
         if (next >= end && !exhausted) {
           // claim the next index range (persistent-thread re-queue)
+          const uint32_t want = claim_size(a.tile, a.tile_min, a.guide_div, n32 - end);
           unsigned long long t = 0;
-          if (lane == 0) t = atomicAdd(a.queue, (unsigned long long)a.tile);
+          if (lane == 0) t = atomicAdd(a.queue, (unsigned long long)want);
           t = __shfl_sync(kFull, t, 0);
           if (t >= (unsigned long long)a.n) { exhausted = true; }
           else {
             next = (uint32_t)t;
-            end = (n32 - next > (uint32_t)a.tile) ? next + (uint32_t)a.tile : n32;
+            end = (n32 - next > want) ? next + want : n32;
           }
         }
         EndTerms et;

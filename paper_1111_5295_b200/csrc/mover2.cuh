@@ -245,13 +245,14 @@ mover2_kernel(const MoverArgs<float> a) {
       const bool go = exhausted ? (n_parked == 64) : (n_parked >= a.refill_threshold);
       if (go) {
         if (next >= end && !exhausted) {
+          const uint32_t want = claim_size(a.tile, a.tile_min, a.guide_div, n32 - end);
           unsigned long long t = 0;
-          if (lane == 0) t = atomicAdd(a.queue, (unsigned long long)a.tile);
+          if (lane == 0) t = atomicAdd(a.queue, (unsigned long long)want);
           t = __shfl_sync(kFull, t, 0);
           if (t >= (unsigned long long)a.n) { exhausted = true; }
           else {
             next = (uint32_t)t;
-            end = (n32 - next > (uint32_t)a.tile) ? next + (uint32_t)a.tile : n32;
+            end = (n32 - next > want) ? next + want : n32;
           }
         }
         EndTerms et0, et1;

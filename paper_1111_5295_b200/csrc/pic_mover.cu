@@ -7,6 +7,28 @@
 #include "mover2.cuh"
 #include "pic_internal.h"
 
+// Guided self-scheduling of the work queue (mover.cuh: claim_size).  A warp claims `tile`
+// (<= 512) particles while plenty are left and (what is left) / (PIC_GUIDE x warps of the grid)
+// towards the end, never fewer than the minimum below: the last ranges are short, so the warps
+// finish together (configs[3]: -4.7 %, configs[4] pass: -9 %, configs[2]: -0.7 %).  Species so
+// small that a warp gets fewer than 192 particles in all (configs[1]) do better with one or two
+// long claims per warp: every claim is a global atomic whose latency the warp waits out.
+#ifndef PIC_GUIDE
+#define PIC_GUIDE 4
+#endif
+#ifndef PIC_GUIDE_MIN
+#define PIC_GUIDE_MIN 32
+#endif
+#ifndef PIC_GUIDE_MIN2
+#define PIC_GUIDE_MIN2 64
+#endif
+#ifndef PIC_TINY_MIN
+#define PIC_TINY_MIN 128
+#endif
+#ifndef PIC_TINY_MIN2
+#define PIC_TINY_MIN2 256
+#endif
+
 namespace picb200 {
 
 namespace {
@@ -97,6 +119,11 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
   a.max_substeps = P.max_substeps;
   a.picard_max = P.picard_max;
   a.tile = S.tile;
+  {
+    const long long warps = (long long)S.grid_blocks * (LaunchCfg<T>::block / 32);
+    a.tile_min = S.n < 192 * warps ? PIC_TINY_MIN : PIC_GUIDE_MIN;
+    a.guide_div = PIC_GUIDE * (uint32_t)warps;
+  }
   a.deposit = (P.flags & PIC_FLAG_NO_DEPOSIT) ? 0 : 1;
   a.wrap_mask = (h->grid.n_cells > 1 && (h->grid.n_cells & (h->grid.n_cells - 1)) == 0)
                     ? h->grid.n_cells - 1 : 0;
@@ -130,6 +157,9 @@ void launch_t(pic_handle* h, SpeciesState& S, const double* dE_n, const double* 
         !(P.flags & PIC_FLAG_ONE_PER_LANE)) {
       a.refill_threshold = (S.nv > 1 || S.nx > 1) ? kRefill2Vsort : kRefill2;
       a.tile = S.tile2;
+      const long long warps2 = (long long)S.grid_blocks2 * (kBlock2 / 32);
+      a.tile_min = S.n < 192 * warps2 ? PIC_TINY_MIN2 : PIC_GUIDE_MIN2;
+      a.guide_div = PIC_GUIDE * (uint32_t)warps2;
       S.last_blocks = S.grid_blocks2;
       h->last_kernel = "mover2_kernel";
       mover2_kernel<<<dim3(S.grid_blocks2), dim3(kBlock2), h->smem_bytes2, h->stream>>>(a);
@@ -191,11 +221,6 @@ int mover_configure(pic_handle* h) {
     S.grid_blocks = (int)std::max<long long>(1, std::min(full, want));
     const long long warps = (long long)S.grid_blocks * (block / 32);
     long long tile = S.n / (warps * 8);                 // >= 8 claims per warp
-// Smallest index range a warp claims from the queue.  Every claim is a global atomic whose
-// latency the warp waits out, so small species (1-4 M particles: fewer than 500 per warp) run
-// faster with a few long claims per warp than with one claim per refill, even though some warps
-// then get no work: 128 (one particle per lane) / 256 (two) measured best on configs[1] and [4]
-// (mover pass 0.104 -> 0.068 ms, 0.189 -> 0.163 ms; profiles/r2_bench.md).
 #ifndef PIC_TILE_MIN
 #define PIC_TILE_MIN 128
 #endif
