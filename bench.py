@@ -36,14 +36,14 @@ UNIT = "sub-steps/s"
 OPS_INCELL, OPS_CROSS = 43.0, 72.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one mover launch from the committed
 # `ncu --set full` capture (profiles/r1_mover_ncu.md); known only for the default workload.
-NCU_TRAFFIC_BYTES = {("cfg2", 100_000_000, "fp32"): 2.365e9, ("cfg2", 100_000_000, "fp64"): 3.966e9}
+NCU_TRAFFIC_BYTES = {("cfg2", 100_000_000, "fp32"): 2.365e9, ("cfg2", 100_000_000, "fp64"): 3.970e9}
 NCU_TRAFFIC_SOURCE = "profiles/r2_mover_ncu.md (ncu --set full capture of this kernel; not measured in this run)"
 # Executed thread-operations per sub-step of the timed kernel, summed over the SASS lines of the
 # same ncu capture (source page, predicated-on thread instructions): (a) the paper's convention
 # (every instruction 1, FFMA 2, packed FFMA2 4, FMUL2 / FADD2 2), (b) floating-point arithmetic
 # only (FADD, FMUL, FFMA, their packed forms; no integer, compare, select, MUFU, memory, control).
-NCU_EXECUTED_OPS = {("cfg2", 100_000_000, "fp32", "mover2_kernel"): (46.07, 27.48),
-                    ("cfg2", 100_000_000, "fp64", "mover_kernel"): (81.01, 46.19)}
+NCU_EXECUTED_OPS = {("cfg2", 100_000_000, "fp32", "mover2_kernel"): (46.12, 27.45),
+                    ("cfg2", 100_000_000, "fp64", "mover_kernel"): (81.22, 46.17)}
 
 
 def _workload(name, n, seed):
