@@ -180,6 +180,31 @@ int pic_set_flags(pic_handle* h, uint32_t flags);
  * reduced on the device in fp64; ke_out[n_species] HOST.  Diagnostic for the energy pin P-9. */
 int pic_kinetic_energy(pic_handle* h, int which, double* ke_out);
 
+/* pic_kinetic_energy_noalloc — the same per-species kinetic energy (sum_p w_m v_p^2 / 2, fp64
+ * sums; the P-9 energy diagnostic a run evaluates every time step) for host programs that must
+ * not allocate GPU memory once their time loop runs: programs whose own pool already holds
+ * (nearly) all of the card's memory, so that even the few bytes pic_kinetic_energy cudaMallocs
+ * per call may be refused; programs with other streams or handles in flight, which the cudaFree
+ * in pic_kinetic_energy would stall (it waits for the whole device); and programs run under a
+ * "no allocation after set-up" rule.  This entry point calls no cudaMalloc / cudaFree / allocating
+ * routine: its block sums go to a fixed 64 KiB device array that is part of the library image
+ * (reserved on every GPU that loads the library, until the process ends).
+ *   ke_out[n_species], HOST (the call then synchronises the handle's stream) or DEVICE (it does
+ *   not).  which = PIC_STATE_N | PIC_STATE_NP1.
+ * Limit: at most PIC_KE_NOALLOC_MAX_SPECIES species per handle (any number of particles);
+ * more -> PIC_ERR_UNSUPPORTED with a message, nothing launched.  The handle must live on the
+ * CURRENT device (else PIC_ERR_ARG).
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, which also
+ * loads the kernels); make it during set-up, before any stream capture on that device.
+ * Sharing: the array is one per GPU, shared by all handles, streams and threads, and keeps the
+ * previous call's contents (every slot a call reads it has written first, so nothing needs
+ * clearing).  Calls whose GPU work can overlap -- different streams without an ordering between
+ * them -- race on it: order them on one stream or with an event.
+ * The partial sums are added in a fixed order: same state, same bits, call after call
+ * (pic_kinetic_energy's atomics give the same value only up to rounding order). */
+enum { PIC_KE_NOALLOC_MAX_SPECIES = 8 };
+int pic_kinetic_energy_noalloc(pic_handle* h, int which, double* ke_out);
+
 /* pic_rho — charge density on cell centres, quadratic B-spline (A-10), of state `which`, all
  * species; rho_out[n_cells] HOST or DEVICE.  Used for Gauss-law initialisation (A-13) and the
  * continuity diagnostic; not on the hot path. */

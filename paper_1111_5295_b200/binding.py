@@ -25,12 +25,14 @@ PIC_FLAG_ONE_PER_LANE = 64
 PIC_FLAG_EXACT_TIME = 128
 PIC_FLAG_STRIDED = 256
 PIC_ERR_SUBSTEP_CAP = -4
+PIC_ERR_UNSUPPORTED = -6
+PIC_KE_NOALLOC_MAX_SPECIES = 8
 
 EXPORTS = ["pic_init", "pic_move_accumulate", "pic_set_step", "pic_residual", "pic_commit",
            "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_set_flags",
            "pic_kinetic_energy", "pic_rho", "pic_jfnk_step", "pic_jfnk_step_dc",
            "pic_copy_state", "pic_destroy", "pic_last_error", "pic_last_kernel", "pic_version", "pic_count_histogram", "pic_microbench",
-           "pic_debug_bounds"]
+           "pic_debug_bounds", "pic_kinetic_energy_noalloc"]
 
 
 class PicGrid(C.Structure):
@@ -268,6 +270,17 @@ class Pic:
     def kinetic_energy(self, which=PIC_STATE_N):
         out = np.empty(self.n_species)
         self._chk(self._L.pic_kinetic_energy(self._h, C.c_int(which), _ptr(out)))
+        return out
+
+    def kinetic_energy_noalloc(self, which=PIC_STATE_N, ke_out=None):
+        """pic_kinetic_energy_noalloc: kinetic_energy() without any device allocation (block sums
+        in the library's static 64 KiB device array), for programs that may not allocate in their
+        time loop.  At most PIC_KE_NOALLOC_MAX_SPECIES species.  ke_out: float64[n_species] numpy
+        array or CUDA tensor to fill (default: a new numpy array).  Calls that can overlap on
+        the GPU share the array and race; make the first call on a device before any capture."""
+        out = np.empty(self.n_species) if ke_out is None else ke_out
+        _check_f64(out, self.n_species, "ke_out")
+        self._chk(self._L.pic_kinetic_energy_noalloc(self._h, C.c_int(which), _ptr(out)))
         return out
 
     def rho(self, which=PIC_STATE_N, rho_out=None):
