@@ -203,6 +203,7 @@ void free_all(pic_handle* h) {
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
+  if (h->ev_pin) cudaEventDestroy(h->ev_pin);
 }
 
 thread_local std::string g_init_err;
@@ -286,6 +287,7 @@ int pic_init(pic_handle** out, const pic_grid* grid, const pic_species* species,
   INIT_CUDA(cudaMemsetAsync(h->d_flag, 0, sizeof(int32_t), h->stream));
   INIT_CUDA(cudaEventCreate(&h->ev0));
   INIT_CUDA(cudaEventCreate(&h->ev1));
+  INIT_CUDA(cudaEventCreateWithFlags(&h->ev_pin, cudaEventDisableTiming));
   h->sp.resize(n_species);
   for (int s = 0; s < n_species; ++s) {
     SpeciesState& S = h->sp[s];
@@ -393,8 +395,20 @@ int pic_set_step(pic_handle* h, const double* E_n, double dt, double tol) {
 
 }  // extern "C"
 
+// h_pin is the source of truly asynchronous H2D copies.  A call that returned without
+// synchronising (host E in, DEVICE residual out) may still have its copy queued -- e.g. behind
+// pic_commit's re-binning kernels -- when the next call wants to overwrite the buffer: that call
+// would then evaluate the residual at the NEXT call's field.  Wait for the pending copy first.
+static int pin_wait(pic_handle* h) {
+  if (h->pin_busy) {
+    PIC_CUDA(h, cudaEventSynchronize(h->ev_pin));
+    h->pin_busy = false;
+  }
+  return PIC_OK;
+}
+
 // One residual evaluation from host E^{n+1} to host R as a CUDA graph, captured once per
-// (flags, dt, tol) and replayed: at 1-4 M particles a pass is 0.1-0.2 ms of kernels, and the five
+// (flags, dt, tol, handle epoch) and replayed: at 1-4 M particles a pass is 0.1-0.2 ms of kernels, and the five
 // launches, two copies and two event records around them were a quarter of its wall time.
 // Returns PIC_ERR_UNSUPPORTED if the stream cannot be captured (the caller falls back).
 static int residual_graph(pic_handle* h, const double* E_np1, double* resid_out) {
@@ -410,7 +424,9 @@ static int residual_graph(pic_handle* h, const double* E_np1, double* resid_out)
   double* out = h->h_pin + (ng + 1);
   pic_handle::ResidualGraph* g = nullptr;
   for (auto& e : h->graphs)
-    if (e.flags == h->params.flags && e.dt == h->step_dt && e.tol == h->step_tol) g = &e;
+    if (e.flags == h->params.flags && e.dt == h->step_dt && e.tol == h->step_tol &&
+        e.epoch == h->epoch)
+      g = &e;
   if (!g) {
     if (h->graphs.size() >= 8) {
       for (auto& e : h->graphs) cudaGraphExecDestroy(e.exec);
@@ -445,9 +461,10 @@ static int residual_graph(pic_handle* h, const double* E_np1, double* resid_out)
       cudaGetLastError();
       return PIC_ERR_UNSUPPORTED;
     }
-    h->graphs.push_back({h->params.flags, h->step_dt, h->step_tol, exec, nl});
+    h->graphs.push_back({h->params.flags, h->step_dt, h->step_tol, exec, nl, h->epoch});
     g = &h->graphs.back();
   }
+  if (int rc = pin_wait(h)) return rc;
   std::memcpy(h->h_pin, E_np1, sizeof(double) * ng);
   PIC_CUDA(h, cudaGraphLaunch(g->exec, st));
   h->launches += g->n_launches;
@@ -479,8 +496,13 @@ int picb200::residual_impl(pic_handle* h, const double* E_np1, double* resid_out
     h->graphs_off = true;     // capture not possible here: plain launches
   }
   if (!e_dev) {
+    if ((rc = pin_wait(h)) != PIC_OK) return rc;
     std::memcpy(h->h_pin, E_np1, sizeof(double) * ng);
     PIC_CUDA(h, cudaMemcpyAsync(h->dE_np1, h->h_pin, sizeof(double) * ng, cudaMemcpyHostToDevice, h->stream));
+    if (r_dev) {   // this call will not synchronise: remember that the copy may still be pending
+      PIC_CUDA(h, cudaEventRecord(h->ev_pin, h->stream));
+      h->pin_busy = true;
+    }
     dEp = h->dE_np1;
   }
   if ((rc = move_device(h, h->dE_step, dEp, h->step_dt, h->step_tol)) != PIC_OK) return rc;
@@ -543,6 +565,11 @@ int pic_copy_state(pic_handle* dst, pic_handle* src) {
   }
   PIC_CUDA(dst, cudaGetLastError());
   dst->have_np1 = false;
+  // the sort key (nx, nv, strided) feeds launch arguments that captured residual graphs hold by
+  // value (refill threshold): graphs of the old key are stale from here on
+  dst->epoch++;
+  for (auto& e : dst->graphs) cudaGraphExecDestroy(e.exec);
+  dst->graphs.clear();
   return PIC_OK;
 }
 

@@ -248,6 +248,7 @@ int pic_destroy(pic_handle* h) {
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
+  if (h->ev_pin) cudaEventDestroy(h->ev_pin);
   delete h;
   return PIC_OK;
 }

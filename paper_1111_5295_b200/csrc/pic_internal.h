@@ -60,6 +60,8 @@ struct pic_handle {
   unsigned long long* d_queue = nullptr;  // [n_species] + [ST_COUNT]: one allocation, one memset
   unsigned long long* d_stats = nullptr;  // = d_queue + n_species
   double* h_pin = nullptr;                // pinned host staging, 2 x (n_cells + 1)
+  cudaEvent_t ev_pin = nullptr;           // recorded after an H2D copy out of h_pin that no
+  bool pin_busy = false;                  // synchronisation follows: wait before h_pin is rewritten
   int32_t* d_hist = nullptr;              // [n_keys + 1] binning scratch
   long long n_keys = 0;
   int32_t* d_scan = nullptr;              // [n_keys / 4096 + 1] chunk sums of the scan
@@ -71,10 +73,13 @@ struct pic_handle {
     double dt, tol;
     cudaGraphExec_t exec;
     long long n_launches;
+    long long epoch;                   // handle epoch the kernel arguments were captured in
   };
   std::vector<ResidualGraph> graphs;
   cudaStream_t own_stream = nullptr;   // for graph launches when `stream` is the legacy default stream
   bool graphs_off = false;             // a capture failed once: plain launches from then on
+  long long epoch = 0;                 // bumped by whatever changes launch arguments a graph bakes
+                                       // in besides (flags, dt, tol): pic_copy_state (sort key)
   pic_stats stats{};
   long long launches = 0;
   const char* last_kernel = "";   // name of the mover kernel of the last launch

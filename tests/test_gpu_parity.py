@@ -509,3 +509,81 @@ def test_energy_identity_on_gpu(G):
         print(f"[energy] {precision}: dK={dK:.6e} work={work:.6e} rel={(dK - work) / abs(work):.2e}")
         assert abs(dK - work) <= tol * abs(work)
         pic.close()
+
+
+def test_residual_host_in_device_out_back_to_back(G):
+    """pic_residual with a HOST field and a DEVICE residual returns without synchronising, and its
+    field goes to the device through the handle's one pinned staging buffer.  Two such calls in a
+    row, issued while the stream is still busy with earlier work, must each see their OWN field:
+    the second call has to wait for the first call's copy before it rewrites the buffer
+    (pic_api.cu: pin_wait)."""
+    import torch
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config2(n=400_000)
+    ng, dt = cfg["n_cells"], cfg["dt"]
+    pic = B.Pic(ng, cfg["length"], cfg["species"], precision="fp32",
+                stream=torch.cuda.current_stream().cuda_stream)
+    pic.set_step(cfg["E_n"], dt)
+    E1 = np.ascontiguousarray(cfg["E_np1"])
+    E2 = np.ascontiguousarray(1.5 * cfg["E_np1"] + 0.01 * np.cos(2 * np.pi * np.arange(ng) / ng))
+    R1, R2 = pic.residual(E1).copy(), pic.residual(E2).copy()      # host in, host out
+    assert G.rel_l2(R1, R2) > 1e-3                                 # the two fields tell apart
+    busy = torch.empty(1 << 28, dtype=torch.float32, device="cuda")   # 1 GiB
+    d1 = torch.empty(ng, dtype=torch.float64, device="cuda")
+    d2 = torch.empty(ng, dtype=torch.float64, device="cuda")
+    for rep in range(3):
+        for _ in range(12):
+            busy.fill_(float(rep))              # a few ms of queued work ahead of the copies
+        pic.residual(E1, resid_out=d1)          # host in, device out: no synchronisation
+        pic.residual(E2, resid_out=d2)
+        torch.cuda.synchronize()
+        assert G.rel_l2(d1.cpu().numpy(), R1) < 1e-9, rep
+        assert G.rel_l2(d2.cpu().numpy(), R2) < 1e-9, rep
+    # and the host/host path right after a device-out call (same staging buffer, graph replay)
+    for _ in range(12):
+        busy.fill_(7.0)
+    pic.residual(E1, resid_out=d1)
+    assert G.rel_l2(pic.residual(E2), R2) < 1e-9
+    torch.cuda.synchronize()
+    assert G.rel_l2(d1.cpu().numpy(), R1) < 1e-9
+    pic.close()
+
+
+def test_residual_graph_not_stale_after_copy_state(G, oracle):
+    """The host/host pic_residual is a CUDA graph replayed per (flags, dt, tol).  pic_copy_state
+    gives the handle another state AND another sort key (here: the paper's strided order instead
+    of the cell-major one), which changes launch arguments the graph holds by value: the next
+    pic_residual must be captured afresh (handle epoch) and agree with the oracle from the new
+    state and with the plain-launch path (device pointers) of the same handle."""
+    import torch
+    from paper_1111_5295_b200 import binding as B
+    cfg = W.config0()
+    sp, dt = cfg["species"][0], cfg["dt"]
+    En, Ep = cfg["E_n"], cfg["E_np1"]
+    ref = G.oracle_run(oracle, cfg)
+    r1 = ref["species"][0]
+    src = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp64",
+                flags=B.PIC_FLAG_VSORT | B.PIC_FLAG_STRIDED)
+    src.move_accumulate(En, Ep, dt)
+    src.commit()                                   # src's state n = the oracle's state n+1
+    dst = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp64", flags=B.PIC_FLAG_VSORT)
+    dst.set_step(Ep, dt)
+    Ra = dst.residual(Ep).copy()                   # captured from the initial state
+    refa = G.oracle_run(oracle, dict(cfg, E_n=Ep))
+    assert G.rel_l2(Ra, oracle.residual(Ep, Ep, dt, refa["jbar"])) < 1e-10
+    n0 = dst.get_stats()["n_launches"]
+    dst.copy_state_from(src)
+    Rb = dst.residual(Ep).copy()
+    refb = G.oracle_run(oracle, dict(cfg, E_n=Ep), state=[(r1["cell"], r1["s"], r1["v"])])
+    Rb_ref = oracle.residual(Ep, Ep, dt, refb["jbar"])
+    assert G.rel_l2(Rb, Rb_ref) < 1e-9
+    assert G.rel_l2(Ra, Rb) > 1e-6                 # the two states tell apart
+    assert dst.get_stats()["n_launches"] > n0
+    dE = torch.from_numpy(Ep).cuda()
+    dR = torch.empty(cfg["n_cells"], dtype=torch.float64, device="cuda")
+    dst.residual(dE, resid_out=dR)                 # plain launches, arguments packed now
+    torch.cuda.synchronize()
+    assert G.rel_l2(dR.cpu().numpy(), Rb) < 1e-12
+    assert G.rel_l2(dst.residual(Ep), Rb) < 1e-12  # replay of the new graph
+    src.close()
+    dst.close()
