@@ -212,8 +212,14 @@ int pic_rho(pic_handle* h, int which, double* rho_out);
 
 /* pic_jfnk_step — one fully implicit time step (north_star (c); S8(f) #1):
  * host fp64 Newton + restarted GMRES on E^{n+1} with the GPU mover as the residual, particles
- * enslaved.  E (HOST, n_cells) holds E^n on entry and E^{n+1} on return; on convergence the
- * particle state is committed.  info (may be NULL) receives iteration counts. */
+ * enslaved.  E (HOST, n_cells) holds E^n on entry.  Returns PIC_OK when the step is accepted: E
+ * then holds E^{n+1} and the particle state n+1 has been committed (pic_commit) -- the two always
+ * change together.  A rejected step changes neither: PIC_ERR_STATE if Newton did not reach
+ * rtol/atol within max_newton, PIC_ERR_SUBSTEP_CAP if it converged but orbits of the converged
+ * state were cut off at max_substeps (A-9; unlike pic_move_accumulate, whose truncated jbar is
+ * still written, a truncated state is never committed); E is then still E^n, the particles are at
+ * state n, and the call can be repeated with other settings.  info (may be NULL) receives the
+ * iteration counts and residual norms in every case. */
 typedef struct pic_jfnk_opts {
   double rtol;             /* nonlinear relative tolerance ||R|| <= rtol ||R_0||                */
   double atol;             /* nonlinear absolute tolerance                                     */

@@ -178,13 +178,17 @@ int jfnk_core(pic_handle* h, pic_handle* hj, double* E, double dt, double tol,
     info->resid0 = r0;
     info->resid = rn;
   }
-  for (int i = 0; i < n; ++i) E[i] = Ek[i];
+  // A rejected step leaves the caller where it was: E still holds E^n and the particles are at
+  // state n, so the step can be retried (smaller dt, larger max_substeps); E^{n+1} is delivered
+  // only together with the committed particle state.
   if (!conv)
-    return set_err(h, PIC_ERR_STATE, "pic_jfnk_step: Newton did not converge (state not committed)");
+    return set_err(h, PIC_ERR_STATE,
+                   "pic_jfnk_step: Newton did not converge (E left at E^n, state not committed)");
   if (capped)   // A-9: some orbits of the converged state did not use up dt
     return set_err(h, PIC_ERR_SUBSTEP_CAP,
-                   "pic_jfnk_step: particles cut off at max_substeps (state not committed)");
+                   "pic_jfnk_step: particles cut off at max_substeps (E left at E^n, state not committed)");
   if ((rc = pic_commit(h)) != PIC_OK) return rc;
+  for (int i = 0; i < n; ++i) E[i] = Ek[i];
   if (dc) return pic_copy_state(hj, h);   // the Jacobian handle follows the committed state
   return PIC_OK;
 }

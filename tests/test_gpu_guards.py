@@ -140,3 +140,65 @@ def test_crossing_clamps(G, oracle, precision, kind):
         t = G.TOL[precision]
         assert max(m["x"]) <= t["x"] and m["j"] <= t["j"] and m["cont"] <= t["cont"]
     m["gpu"]["pic"].close()
+
+
+def _raw_jfnk(pic, E, dt, **kw):
+    """pic_jfnk_step through the bare C call: (rc, info) without the binding's exception."""
+    from paper_1111_5295_b200 import binding as B
+    o = dict(rtol=1e-8, atol=0.0, fd_eps=0.0, gmres_rtol=1e-2, max_newton=20, gmres_restart=30,
+             max_gmres=200)
+    o.update(kw)
+    opts = B.PicJfnkOpts(o["rtol"], o["atol"], o["fd_eps"], o["gmres_rtol"], o["max_newton"],
+                         o["gmres_restart"], o["max_gmres"], 0)
+    info = B.PicJfnkInfo()
+    rc = pic._L.pic_jfnk_step(pic._h, B._ptr(E), B.C.c_double(dt), B.C.c_double(1e-10),
+                              B.C.byref(opts), B.C.byref(info))
+    return rc, info.as_dict()
+
+
+def test_jfnk_rejected_step_changes_nothing():
+    """include/pic.h, pic_jfnk_step: E^{n+1} is delivered only together with the committed state.
+    A step that is rejected -- Newton short of rtol (PIC_ERR_STATE), or converged on orbits that
+    were cut off at max_substeps (PIC_ERR_SUBSTEP_CAP, A-9) -- leaves E at E^n and the particles
+    at state n; the same handle then still takes an acceptable step."""
+    from paper_1111_5295_b200 import binding as B
+    from paper_1111_5295_b200 import workloads as W
+    cfg = W.config1(ppc=40)                      # IAW, 256 cells, 2 x 10,240 particles
+    dt = cfg["dt"]
+    E0 = np.ascontiguousarray(cfg["E_n"])
+
+    def state(pic):
+        return [pic.get_particles(s, B.PIC_STATE_N) for s in range(pic.n_species)]
+
+    def same(a, b):
+        return all(np.array_equal(p["cell"], q["cell"]) and np.array_equal(p["xi"], q["xi"]) and
+                   np.array_equal(p["v"], q["v"]) for p, q in zip(a, b))
+
+    # (1) not converged: one Newton step cannot reach 1e-13
+    pic = B.Pic(cfg["n_cells"], cfg["length"], cfg["species"], precision="fp64")
+    s0 = state(pic)
+    E = E0.copy()
+    rc, info = _raw_jfnk(pic, E, dt, rtol=1e-13, max_newton=1)
+    assert rc == -5 and info["converged"] == 0 and info["newton_its"] == 1, (rc, info)
+    assert info["resid"] < info["resid0"]        # the iterate did move ...
+    assert np.array_equal(E, E0)                 # ... but the caller's field did not
+    assert same(state(pic), s0)
+    # the same handle, acceptable settings: accepted, E and the state change together
+    rc, info = _raw_jfnk(pic, E, dt, rtol=1e-8)
+    assert rc == 0 and info["converged"] == 1, (rc, info)
+    assert not np.array_equal(E, E0) and not same(state(pic), s0)
+    pic.close()
+
+    # (2) converged on truncated orbits: dt = 100 needs a hundred and more sub-steps per electron,
+    # the cap is 16 (the kernel tests it every 64 sub-steps); a loose rtol is met after >= 1 update
+    pic = B.Pic(cfg["n_cells"], cfg["length"], cfg["species"], precision="fp64", max_substeps=16)
+    s0 = state(pic)
+    E = E0.copy()
+    rc, info = _raw_jfnk(pic, E, 100.0, rtol=0.5, max_newton=10)
+    print(f"[guards] jfnk on capped orbits: rc={rc} {info}")
+    assert rc == B.PIC_ERR_SUBSTEP_CAP and info["converged"] == 1 and info["newton_its"] >= 1, (rc, info)
+    assert b"not committed" in pic._L.pic_last_error(pic._h)
+    assert pic.get_stats()["n_substep_cap"] > 0
+    assert np.array_equal(E, E0)
+    assert same(state(pic), s0)
+    pic.close()
