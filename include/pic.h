@@ -35,7 +35,9 @@ typedef enum pic_status {
   PIC_ERR_PARTICLE = -3,   /* pic_init: a particle has non-finite x or v, or x outside [0,L) */
   PIC_ERR_SUBSTEP_CAP = -4,/* a particle hit max_substeps (A-9); results are still written   */
   PIC_ERR_STATE = -5,      /* call order: pic_residual before pic_set_step, commit before move */
-  PIC_ERR_UNSUPPORTED = -6 /* per-visit deposit asked for on a grid too large for shared memory */
+  PIC_ERR_UNSUPPORTED = -6 /* per-visit deposit or (fp32) exact time accounting asked for on a grid
+                              too large for shared memory, at pic_init or pic_set_flags; more
+                              species than pic_kinetic_energy_noalloc holds                    */
 } pic_status;
 
 enum { PIC_FP32 = 0, PIC_FP64 = 1 };   /* arithmetic of the mover kernel (north_star (b))    */
@@ -60,7 +62,10 @@ enum {
                               class, instead of sharing a cell (A/B of S8(f) #3; same results)   */
   PIC_FLAG_EXACT_TIME = 128, /* fp32 only: exact accounting of the time used by the sub-steps
                               (fp64 checkpoints of the remaining time, D:5) instead of a plain
-                              fp32 `r -= dtau`, whose rounding random-walks to ~ulp(dt) sqrt(n_sub) */
+                              fp32 `r -= dtau`, whose rounding random-walks to ~ulp(dt) sqrt(n_sub);
+                              runs the one-particle-per-lane kernel (the packed two-per-lane one
+                              has no such variant); ignored by fp64 handles, whose r is exact
+                              enough; PIC_ERR_UNSUPPORTED on grids beyond shared memory          */
   PIC_FLAG_DEPOSIT_PER_VISIT = 16 /* deposit per cell visit with shared fp64 atomics
                               instead of the default end-point form (D:5); same jbar to rounding */
 };
@@ -173,7 +178,9 @@ int pic_count_histogram(pic_handle* h, int species, uint32_t bin_width, int32_t 
 int pic_get_stats(pic_handle* h, pic_stats* out);
 
 /* pic_set_flags — replace pic_params.flags (COUNTS / DIAG / NO_STORE / NO_DEPOSIT /
- * ONE_PER_LANE / DEPOSIT_PER_VISIT) between calls. */
+ * ONE_PER_LANE / DEPOSIT_PER_VISIT / EXACT_TIME) between calls.  PIC_ERR_UNSUPPORTED (flags
+ * unchanged) for DEPOSIT_PER_VISIT or fp32 EXACT_TIME on a grid too large for shared memory;
+ * PIC_ERR_STATE for COUNTS on a handle created without it (no buffers). */
 int pic_set_flags(pic_handle* h, uint32_t flags);
 
 /* pic_kinetic_energy — sum_p w_m v_p^2 / 2 per species (w_m = w_q / (q/m)) of state `which`,

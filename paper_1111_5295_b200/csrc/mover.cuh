@@ -402,6 +402,45 @@ __device__ __forceinline__ void block_flush(const MoverArgs<T>& a, const double*
   }
 }
 
+// The same flush for the GGRID instantiation, whose "shared" grid copy is a row of GLOBAL memory
+// that the block's warps have been updating with atomics (performed in L2).  Two differences:
+// the faces are taken in tiles of blockDim.x with thread t on face base + t, so that a warp reads
+// and writes 32 consecutive elements (contiguous per-thread chunks cost one memory transaction
+// per lane), with a running carry from tile to tile; and sF / sD are read with ld.global.cg
+// (__ldcg, L2), never through a possibly stale L1 line or a read-only path.  (The __restrict__
+// qualifiers of the helpers above only promise that nothing else writes the arrays while that
+// helper runs, which holds; the compiler does not turn them into non-coherent loads -- no
+// LDG.CONSTANT in any mover_kernel instantiation -- but this path does not depend on it.)
+template <typename T>
+__device__ __forceinline__ void block_flush_global(const MoverArgs<T>& a, const double* sF,
+                                                   const int32_t* sD, int32_t* s_wtot) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (int)blockDim.x >> 5;
+  __syncthreads();
+  double* row = a.partial + (size_t)blockIdx.x * a.n_cells;
+  int32_t carry = 0;                             // sum of sD over the faces of earlier tiles
+  for (int base = 0; base < a.n_cells; base += (int)blockDim.x) {
+    const int f = base + (int)threadIdx.x;
+    const int32_t d = f < a.n_cells ? __ldcg(sD + f) : 0;
+    int32_t inc = d;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int32_t t = __shfl_up_sync(kFull, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_wtot[wid] = inc;
+    __syncthreads();
+    int32_t run = carry + inc, tot = 0;          // inclusive prefix sum up to face f
+    for (int w = 0; w < nw; ++w) {
+      const int32_t t = s_wtot[w];
+      if (w < wid) run += t;
+      tot += t;
+    }
+    if (f < a.n_cells) row[f] = a.scale * (__ldcg(sF + f) + (double)run);
+    carry += tot;
+    __syncthreads();                             // s_wtot is rewritten by the next tile
+  }
+}
+
 // One sub-step (O3-O8) of the lane's particle: estimate dtau, tentative Crank-Nicolson step in
 // the current cell, accept it if it stays in the cell, otherwise truncate it at the face.
 // CN_DIRECT: Eq. 11, else Picard on Eq. 9-10.  The max_substeps cap (A-9) is checked by the
@@ -684,7 +723,8 @@ mover_kernel(const MoverArgs<T> a) {
     if (lane == 0 && v) atomicAdd(&a.stats[i], (unsigned long long)v);
   }
 
-  block_flush<T>(a, sF, sD, s_wtot);
+  if constexpr (GGRID) block_flush_global<T>(a, sF, sD, s_wtot);
+  else block_flush<T>(a, sF, sD, s_wtot);
 }
 
 }  // namespace picb200

@@ -155,6 +155,14 @@ int pic_set_flags(pic_handle* h, uint32_t flags) {
   if (!h) return PIC_ERR_ARG;
   if ((flags & PIC_FLAG_COUNTS) && !h->sp.empty() && !h->sp[0].nsub)
     return set_err(h, PIC_ERR_STATE, "PIC_FLAG_COUNTS must be set at pic_init (buffers)");
+  // the global-memory-grid kernels (grids beyond a block's shared memory) exist with the
+  // end-point deposit and plain fp32 time accounting only: say so instead of ignoring the request
+  if (h->d_grid_scratch) {
+    if (flags & PIC_FLAG_DEPOSIT_PER_VISIT)
+      return set_err(h, PIC_ERR_UNSUPPORTED, "pic_set_flags: per-visit deposit needs the grid in shared memory (n_cells too large)");
+    if ((flags & PIC_FLAG_EXACT_TIME) && h->elem == 4)
+      return set_err(h, PIC_ERR_UNSUPPORTED, "pic_set_flags: exact time accounting is not built for grids beyond shared memory (n_cells too large)");
+  }
   h->params.flags = flags;
   return PIC_OK;
 }

@@ -199,6 +199,8 @@ int mover_configure(pic_handle* h) {
   if (ggrid) {
     if (h->params.flags & PIC_FLAG_DEPOSIT_PER_VISIT)
       return set_err(h, PIC_ERR_UNSUPPORTED, "per-visit deposit needs the grid in shared memory (n_cells too large)");
+    if ((h->params.flags & PIC_FLAG_EXACT_TIME) && h->elem == 4)
+      return set_err(h, PIC_ERR_UNSUPPORTED, "exact time accounting is not built for grids beyond shared memory (n_cells too large)");
     h->grid_stride = (bytes + 255) & ~(size_t)255;
     // one wave of blocks, but no more rows of scratch than ~2 GB
     const size_t budget = (size_t)2 << 30;
