@@ -125,25 +125,35 @@ def landing_cfg(kind, n_cells=4096, dt=1.0, seed=3, q_over_m=-1.0):
     return cfg, [(cells, s0, v0)], (X1, v0 + a * dt)
 
 
-def ulp_response(o, cfg, seed=1):
-    """How much the METHOD amplifies one fp32 rounding error (cfg3): run the oracle
-    (fp64) twice from fp32-representable inputs that differ by one fp32 ulp in every particle's
-    velocity (random sign), and return the relative L2 response of x, v (over the particles that
-    took the same branches) and jbar, plus the mean sub-steps per particle.  An fp32 kernel makes
-    such an error at every one of its n_sub sub-steps, so its distance from the oracle is about
-    response x sqrt(n_sub) (random walk) whatever its arithmetic."""
+def ulp_response(o, cfg, seed=1, fp64=False):
+    """How much the METHOD amplifies one rounding error (cfg3): run the oracle
+    (fp64) twice from inputs that differ by one ulp in every particle's velocity (random sign) --
+    one fp32 ulp from fp32-representable inputs, or with fp64=True one fp64 ulp from the fp64
+    inputs -- and return the relative L2 response of x, v (over the particles that took the same
+    branches) and jbar, the max-norm responses in the units of the parity metrics (xi_max: cells,
+    v_max: relative to the rms speed), plus the mean sub-steps per particle.  A kernel of that
+    precision makes such an error at every one of its n_sub sub-steps, so its distance from the
+    oracle is about response x sqrt(n_sub) (random walk) whatever its arithmetic."""
     dx = cfg["length"] / cfg["n_cells"]
     rng = np.random.default_rng(seed)
     st0, st1 = [], []
-    for r in round_to_fp32_state(cfg):
-        s = r["xi"].astype(np.float64) * dx
-        toward = np.where(rng.random(r["v"].size) < 0.5, -np.inf, np.inf).astype(np.float32)
-        v1 = np.nextafter(r["v"], toward)
-        st0.append((r["cell"], s, r["v"].astype(np.float64)))
-        st1.append((r["cell"], s, v1.astype(np.float64)))
+    if fp64:
+        for sp in cfg["species"]:
+            c, s = o.bin_particles(cfg["n_cells"], cfg["length"], sp["x"])
+            v0 = np.asarray(sp["v"], np.float64)
+            toward = np.where(rng.random(v0.size) < 0.5, -np.inf, np.inf)
+            st0.append((c, s, v0))
+            st1.append((c, s, np.nextafter(v0, toward)))
+    else:
+        for r in round_to_fp32_state(cfg):
+            s = r["xi"].astype(np.float64) * dx
+            toward = np.where(rng.random(r["v"].size) < 0.5, -np.inf, np.inf).astype(np.float32)
+            v1 = np.nextafter(r["v"], toward)
+            st0.append((r["cell"], s, r["v"].astype(np.float64)))
+            st1.append((r["cell"], s, v1.astype(np.float64)))
     p = o.make_params(cn_mode=o.DIRECT)
     a, b = oracle_run(o, cfg, p, state=st0), oracle_run(o, cfg, p, state=st1)
-    out = dict(x=0.0, v=0.0, flips=0)
+    out = dict(x=0.0, v=0.0, flips=0, xi_max=0.0, v_max=0.0)
     for ra, rb in zip(a["species"], b["species"]):
         same = (ra["n_sub"] == rb["n_sub"]) & (ra["n_cross"] == rb["n_cross"]) & \
                (ra["cell"] == rb["cell"])
@@ -152,6 +162,9 @@ def ulp_response(o, cfg, seed=1):
         d = periodic_dist(xa[same], (rb["cell"] * dx + rb["s"])[same], cfg["length"])
         out["x"] = max(out["x"], float(np.linalg.norm(d) / np.linalg.norm(xa[same])))
         out["v"] = max(out["v"], rel_l2(rb["v"][same], ra["v"][same]))
+        vrms = float(np.sqrt(np.mean(ra["v"] ** 2)))
+        out["xi_max"] = max(out["xi_max"], float(d.max() / dx))
+        out["v_max"] = max(out["v_max"], float(np.max(np.abs(rb["v"][same] - ra["v"][same])) / vrms))
     out["j"] = rel_l2(b["jbar"], a["jbar"])
     n = sum(r["n_sub"].size for r in a["species"])
     out["n_sub_mean"] = a["stats"].n_sub / n

@@ -110,9 +110,12 @@ def test_cfg4_first_steps_against_the_oracle(oracle):
     # hybrid at its looser tolerance
     assert o["max_energy_change_per_step"] < 1e-9 and g64["max_energy_change_per_step"] < 1e-9
     assert g32["max_energy_change_per_step"] < 5e-6
-    # local charge conservation (Gauss's law stays satisfied): exact for both precisions, since
-    # the deposit is an exact function of the stored end points
+    # Gauss's law.  Continuity is exact per step in both precisions (the deposit is an exact
+    # function of the stored end points), but E advances by Ampere's law only to the
+    # nonlinear tolerance, so div E - rho picks up the left-over residual of every step: 1e-7 of
+    # |rho| at rtol 1e-8, and for the fp32 run (rtol 2e-4, 20 steps) 2e-3 -- gated at 5e-3
     assert o["max_gauss"] < 1e-6 and g64["max_gauss"] < 1e-6
+    assert g32["max_gauss"] < 5e-3
     # the fp32 hybrid tracks the oracle's macroscopic quantities to its tolerance
     assert g32["ke_e_rel_diff_vs_oracle_last"] < 1e-4
     assert g32["field_energy_rel_diff_vs_oracle_last"] < 5e-3

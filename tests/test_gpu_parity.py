@@ -68,7 +68,20 @@ def test_cfg3_small_invariants(G, oracle, precision):
     m = G.parity(oracle, cfg, precision)
     _report(f"cfg3/20k {precision}", m)
     if precision == "fp64":
+        # L2 bars: north_star's.  Max norms: the generic 1e-8 gates assume a 100-fold tail over
+        # the L2 figure; on these orbits the tail is the orbits' own (a few of them amplify an
+        # error a hundred times more than the average one), so the bar is derived from the
+        # oracle's MAX-norm response to one fp64 ulp: an fp64 kernel rounds about ten times per
+        # sub-step on the way to (x, v) (Eq. 11's denominator and quotient, the two updates, the
+        # remaining time; discriminant, root and quotient on a crossing), a random walk of
+        # 10 n_sub such errors, times 3 for the spread of the estimate.
         G.assert_parity(m, "fp64", max_flip_frac=5e-3, max_norms=False)
+        r = ulp_response(oracle, cfg, fp64=True)
+        k = 3.0 * math.sqrt(10.0 * r["n_sub_mean"])
+        print(f"[parity] cfg3 fp64 derived max-norm bars: xi {k * r['xi_max']:.2e} cells "
+              f"(got {max(m['xi_max']):.2e}), v {k * r['v_max']:.2e} (got {max(m['v_max']):.2e}); "
+              f"L2 estimates x {k * r['x']:.1e} v {k * r['v']:.1e}")
+        assert max(m["xi_max"]) <= k * r["xi_max"] and max(m["v_max"]) <= k * r["v_max"]
     else:
         r = ulp_response(oracle, cfg)
         k = 3.0 * math.sqrt(r["n_sub_mean"])
@@ -78,10 +91,13 @@ def test_cfg3_small_invariants(G, oracle, precision):
         assert m["cont"] <= G.TOL["fp32"]["cont"]
         assert m["flips"] <= 0.05 * m["n"]
         m["gpu"]["pic"].close()
-        # exact time accounting: same orbits to within the same tolerance, no better
+        # exact time accounting: same orbits to within the same tolerance (so far it has not
+        # come out better either -- reported, not required: a better kernel must not fail here)
         m2 = G.parity(oracle, cfg, precision, extra_flags=B.PIC_FLAG_EXACT_TIME)
         _report("cfg3/20k fp32 exact-time", m2)
-        assert max(m2["v"]) <= k * r["v"] and max(m2["v"]) > 0.3 * max(m["v"])
+        print(f"[parity] cfg3 fp32 exact-time / plain: v {max(m2['v']) / max(m['v']):.2f} "
+              f"x {max(m2['x']) / max(m['x']):.2f}")
+        assert max(m2["v"]) <= k * r["v"] and max(m2["x"]) <= k * r["x"]
         m = m2
     assert m["stats"]["n_substep_cap"] == 0
     m["gpu"]["pic"].close()
@@ -273,6 +289,22 @@ def test_large_grid_global_memory_fallback(G, oracle, precision, n_cells):
         pic.close()
     with pytest.raises(B.PicError):      # the per-visit deposit needs the grid in shared memory
         B.Pic(n_cells, length, cfg["species"], precision=precision, flags=B.PIC_FLAG_DEPOSIT_PER_VISIT)
+    # what the global-memory-grid kernels do not implement is refused, at pic_init and at
+    # pic_set_flags alike, never silently dropped; the refused call leaves the flags as they were
+    if precision == "fp32":
+        with pytest.raises(B.PicError):
+            B.Pic(n_cells, length, cfg["species"], precision=precision, flags=B.PIC_FLAG_EXACT_TIME)
+    pic = B.Pic(n_cells, length, cfg["species"], precision=precision)
+    j0 = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+    bad = [B.PIC_FLAG_DEPOSIT_PER_VISIT] + ([B.PIC_FLAG_EXACT_TIME] if precision == "fp32" else [])
+    for flag in bad:
+        with pytest.raises(B.PicError) as ei:
+            pic.set_flags(flag)
+        assert ei.value.code == B.PIC_ERR_UNSUPPORTED and "too large" in str(ei.value)
+    pic.set_flags(B.PIC_FLAG_NO_STORE)                 # a supported one still goes through
+    j1 = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
+    assert G.rel_l2(j1, j0) < 1e-12
+    pic.close()
 
 
 # ---- Vlasov-Poisson variant: orbits without the current deposit, rho at the end
