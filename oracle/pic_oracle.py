@@ -13,7 +13,14 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "pic_oracle.cpp")
-_LIB = os.path.join(_HERE, "libpic_oracle.so")
+# PIC_ORACLE_SANITIZE=1 (tests/test_oracle_sanitized.py): the same source built with
+# AddressSanitizer + UndefinedBehaviorSanitizer as libpic_oracle_san.so.  Loader switch only --
+# the arithmetic is pic_oracle.cpp's either way; the process must then run under
+# LD_PRELOAD=<libasan.so> (the ASan runtime has to be the first library of the process).
+_SANITIZE = os.environ.get("PIC_ORACLE_SANITIZE", "0") == "1"
+_LIB = os.path.join(_HERE, "libpic_oracle_san.so" if _SANITIZE else "libpic_oracle.so")
+_OPT = (["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined",
+         "-fno-sanitize-recover=all"] if _SANITIZE else ["-O2"])
 
 
 def build(force=False):
@@ -21,8 +28,8 @@ def build(force=False):
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
         return _LIB
-    cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fPIC", "-shared", "-Wall",
-           "-o", _LIB, _SRC]
+    cmd = ["g++"] + _OPT + ["-std=c++17", "-ffp-contract=off", "-fPIC", "-shared", "-Wall",
+                            "-o", _LIB, _SRC]
     subprocess.run(cmd, check=True)
     return _LIB
 
