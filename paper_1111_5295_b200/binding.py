@@ -216,21 +216,25 @@ class Pic:
             pass
 
     # -- C-ABI mirrors
-    def move_accumulate(self, E_n, E_np1, dt, tol=1e-10, jbar_out=None):
-        """pic_move_accumulate -> jbar (numpy float64[n_cells] unless jbar_out is given)."""
+    def move_accumulate(self, E_n, E_np1, dt, tol=1e-10, jbar_out=None, allow_cap=False):
+        """pic_move_accumulate -> jbar (numpy float64[n_cells] unless jbar_out is given).
+        PIC_ERR_SUBSTEP_CAP (orbits cut off at max_substeps: jbar is that of the truncated orbits)
+        raises like every other error; allow_cap=True returns the truncated jbar instead."""
         out = np.empty(self.n_cells) if jbar_out is None else jbar_out
         self._chk(self._L.pic_move_accumulate(self._h, _ptr(E_n), _ptr(E_np1), C.c_double(dt),
                                               C.c_double(tol), _ptr(out)),
-                  allow=(PIC_ERR_SUBSTEP_CAP,))
+                  allow=(PIC_ERR_SUBSTEP_CAP,) if allow_cap else ())
         return out
 
     def set_step(self, E_n, dt, tol=1e-10):
         self._chk(self._L.pic_set_step(self._h, _ptr(E_n), C.c_double(dt), C.c_double(tol)))
 
-    def residual(self, E_np1, resid_out=None):
+    def residual(self, E_np1, resid_out=None, allow_cap=False):
+        """pic_residual -> R (numpy float64[n_cells] unless resid_out is given); allow_cap as in
+        move_accumulate."""
         out = np.empty(self.n_cells) if resid_out is None else resid_out
         self._chk(self._L.pic_residual(self._h, _ptr(E_np1), _ptr(out)),
-                  allow=(PIC_ERR_SUBSTEP_CAP,))
+                  allow=(PIC_ERR_SUBSTEP_CAP,) if allow_cap else ())
         return out
 
     def commit(self):

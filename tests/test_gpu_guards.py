@@ -90,6 +90,24 @@ def test_picard_cap_parity(G, oracle, precision):
     m["gpu"]["pic"].close()
 
 
+def test_picard_cap_fp32_at_the_callers_tolerance(G, oracle):
+    """The same workload with the tolerance left where a caller would put it (1e-10): the oracle
+    iterates against 1e-10, the fp32 kernel against its floor of 4 ulp = 4.8e-7 (a tolerance
+    below a few ulp can never be met in fp32, A-3).  What the floor changes: with
+    picard_max = 2 the oracle now hits the cap on (nearly) every sub-step, the kernel only where
+    its two iterates differ by more than 4.8e-7 relative -- fewer -- and both still end on the
+    SECOND iterate or closer than 4.8e-7 to it, so the orbits agree at the fp32 bars all the same."""
+    from paper_1111_5295_b200 import workloads as W
+    cfg = dict(W.config2(n=50_003), tol=1e-10)
+    op = oracle.make_params(cn_mode=oracle.PICARD, tol=1e-10, picard_max=2)
+    m = G.parity(oracle, cfg, "fp32", "picard", oracle_params=op, pic_kw=dict(picard_max=2))
+    _report("picard-cap fp32, oracle at the caller's tol", m)
+    assert m["ostats"]["n_picard_cap"] > 0.9 * m["ostats"]["n_sub"]
+    assert m["stats"]["n_picard_cap"] <= m["ostats"]["n_picard_cap"]
+    G.assert_parity(m, "fp32", max_flip_frac=5e-3)
+    m["gpu"]["pic"].close()
+
+
 @pytest.mark.parametrize("kind", ["land", "turn"])
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_crossing_clamps(G, oracle, precision, kind):

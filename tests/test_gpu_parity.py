@@ -437,9 +437,15 @@ def test_edge_cases(G, oracle):
         _report(f"edge fp64 {cn}", m)
         G.assert_parity(m, "fp64", max_flip_frac=0.0)
         m["gpu"]["pic"].close()
-    m = G.parity(oracle, cfg, "fp32")
-    assert m["cont"] < 1e-5
-    m["gpu"]["pic"].close()
+    # fp32: the same orbits at north_star's fp32 bars.  Seven particles: one branch flip (a
+    # particle that starts ON a face may round to the other side of a decision) is 14 % of them,
+    # so flips are reported and bounded by one, and the bars are asserted on the others
+    for cn in ("picard", "direct"):
+        m = G.parity(oracle, cfg, "fp32", cn)
+        _report(f"edge fp32 {cn}", m)
+        assert m["flips"] <= 1, m["flips"]
+        G.assert_parity(m, "fp32", max_flip_frac=1.0)
+        m["gpu"]["pic"].close()
     # one cell only: both faces are face 0
     cfg1 = dict(n_cells=1, length=1.0, dt=0.9, tol=1e-12, E_n=np.array([0.3]),
                 E_np1=np.array([0.1]),
@@ -475,13 +481,21 @@ def test_substep_cap_is_reported(G):
     cfg = W.config3(n=2000)
     sp = cfg["species"][0]
     pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp64", max_substeps=16)
-    jbar = np.empty(cfg["n_cells"])            # must outlive the call: the library writes into it
+    # the binding raises on the cap like on any other error ...
     with pytest.raises(B.PicError) as ei:
-        pic._chk(pic._L.pic_move_accumulate(pic._h, B._ptr(cfg["E_n"]), B._ptr(cfg["E_np1"]),
-                                            B.C.c_double(cfg["dt"]), B.C.c_double(1e-10),
-                                            B._ptr(jbar)))
+        pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"])
     assert ei.value.code == B.PIC_ERR_SUBSTEP_CAP
     assert pic.get_stats()["n_substep_cap"] > 0
+    pic.set_step(cfg["E_n"], cfg["dt"])
+    with pytest.raises(B.PicError) as ei:
+        pic.residual(cfg["E_np1"])
+    assert ei.value.code == B.PIC_ERR_SUBSTEP_CAP
+    # ... unless the truncated result is asked for: jbar of the cut-off orbits, as written by the call
+    j = pic.move_accumulate(cfg["E_n"], cfg["E_np1"], cfg["dt"], allow_cap=True)
+    R = pic.residual(cfg["E_np1"], allow_cap=True)
+    assert np.all(np.isfinite(j)) and np.any(j != 0.0)
+    ref = (cfg["E_np1"] - cfg["E_n"]) / cfg["dt"] + j - j.mean()
+    assert np.max(np.abs(R - ref)) <= 1e-12 * np.max(np.abs(ref))
     pic.close()
 
 
