@@ -355,6 +355,123 @@ def run_iaw(args, rank, world, local_rank, explicit_steps):
         dist.destroy_process_group()
 
 
+def _peak_gops(sms, precision, sm_max_mhz):
+    """Derived ALU peak: SMs x lanes x 2 (FMA) x clock, GOp/s."""
+    return sms * (128 if precision == "fp32" else 64) * 2 * sm_max_mhz * 1e-3
+
+
+def extra_iaw_leg(B, torch, workload, precision, steps, warmup, seed, stream, sms, sm_max_mhz):
+    """Bounded leg of the default line: `steps` fully implicit time steps (pic_jfnk_step) of
+    configs[1] / configs[4] at full size after `warmup` untimed ones, each step timed with CUDA
+    events on the library's stream; the numbers `--workload cfg1|cfg4` reports, in short."""
+    from paper_1111_5295_b200.iaw import gauss_field
+    cfg = _workload(workload, 0, seed)
+    ng, L, dt = cfg["n_cells"], cfg["length"], cfg["dt"]
+    dx = L / ng
+    rtol = 1e-8 if precision == "fp64" else 2e-4                    # SURVEY A-14
+    flags = B.PIC_FLAG_VSORT
+    pic = B.Pic(ng, L, cfg["species"], precision=precision, cn_mode="direct", flags=flags, stream=stream)
+    n_p = sum(pic.n)
+    E = gauss_field(pic.rho(B.PIC_STATE_N), dx)
+
+    def energy():   # the diagnostic that allocates nothing: it sits inside the time loop
+        return float(pic.kinetic_energy_noalloc(B.PIC_STATE_N).sum() + 0.5 * dx * np.sum(E * E))
+
+    for _ in range(warmup):
+        info = pic.jfnk_step(E, dt, rtol=rtol)
+        assert info["converged"], info
+    pic.set_flags(flags | B.PIC_FLAG_DIAG)          # exact sub-steps / crossings of one pass
+    pic.move_accumulate(E, E, dt)
+    exact = pic.get_stats()
+    pic.set_flags(flags)
+    l0 = pic.get_stats()["n_launches"]
+    e_start = e_prev = energy()
+    ms, hist, drift = [], [], []
+    for _ in range(steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        info = pic.jfnk_step(E, dt, rtol=rtol)
+        b.record()
+        torch.cuda.synchronize()
+        assert info["converged"], info
+        ms.append(a.elapsed_time(b))
+        hist.append(info)
+        e_now = energy()
+        drift.append(abs(e_now - e_prev) / e_start)
+        e_prev = e_now
+    launches = pic.get_stats()["n_launches"] - l0
+    kms = []
+    for _ in range(3):
+        pic.move_accumulate(E, E, dt)
+        kms.append(pic.get_stats()["last_move_ms"])
+    k_ms = float(np.mean(kms))
+    kernel = pic.last_kernel()
+    pic.close()
+    n_sub, n_cross = exact["n_sub"], exact["n_cross"]
+    passes = float(np.mean([h["mover_calls"] for h in hist]))
+    ops = OPS_INCELL * (n_sub - n_cross) + OPS_CROSS * n_cross
+    peak = _peak_gops(sms, precision, sm_max_mhz)
+    mean_ms = float(np.mean(ms))
+    return {"workload": f"{workload}: ion acoustic wave, {ng} cells, "
+                        f"{'+'.join(str(n) for n in pic.n)} particles, dt={dt}, full implicit step",
+            "precision": precision, "jfnk_rtol": rtol, "steps": steps, "warmup": warmup,
+            "ms_per_step": mean_ms, "ms_per_step_min": float(np.min(ms)),
+            "ms_per_step_median": float(np.median(ms)), "ms_per_step_max": float(np.max(ms)),
+            "value": n_sub * passes / (mean_ms * 1e-3), "unit": UNIT,
+            "newton_its_mean": float(np.mean([h["newton_its"] for h in hist])),
+            "gmres_its_mean": float(np.mean([h["gmres_its"] for h in hist])),
+            "mover_passes_mean": passes, "mover_ms_per_pass": k_ms,
+            "mover_share_of_step": k_ms * passes / mean_ms,
+            "substeps_per_particle_per_pass": n_sub / max(n_p, 1),
+            "crossing_fraction": n_cross / max(n_sub, 1),
+            "energy_rel_change_per_step_max": float(np.max(drift)),
+            "energy_rel_change_total": (e_prev - e_start) / e_start,
+            "gpu_launches": int(launches), "kernel": kernel,
+            "roofline_frac_pass": ops / (k_ms * 1e-3) * 1e-9 / peak}
+
+
+def extra_cfg3_leg(B, torch, seed, stream, sms, sm_max_mhz, timed=5, warmup=3):
+    """Bounded leg of the default line: configs[3] (2e7 two-stream particles, dt = 50, the
+    divergence stress case) in fp32: one counting step for the exact sub-step counts and their
+    percentiles, then `timed` launches of the fast build timed by the library's events."""
+    cfg = _workload("cfg3", 0, seed)
+    sp = cfg["species"][0]
+    n_p = sp["x"].shape[0]
+    flags = B.PIC_FLAG_VSORT
+    pic = B.Pic(cfg["n_cells"], cfg["length"], [sp], precision="fp32", cn_mode="direct",
+                flags=flags | B.PIC_FLAG_COUNTS, stream=stream)
+    dEn = torch.from_numpy(cfg["E_n"]).cuda()
+    dEp = torch.from_numpy(cfg["E_np1"]).cuda()
+    dj = torch.empty(cfg["n_cells"], dtype=torch.float64, device="cuda")
+    dt, tol = cfg["dt"], cfg.get("tol", 1e-10)
+    pic.set_flags(flags | B.PIC_FLAG_COUNTS | B.PIC_FLAG_DIAG)
+    pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+    exact = pic.get_stats()
+    mean = exact["n_sub"] / max(n_p, 1)
+    width = max(1, int(math.ceil(2.0 * mean / 64)))
+    hs, _ = pic.count_histogram(0, width, 65)
+    cum = np.cumsum(hs) / max(int(hs.sum()), 1)
+    pct = {str(q): int((np.searchsorted(cum, q / 100.0) + 1) * width) for q in (50, 90, 99)}
+    pic.set_flags(flags)
+    kms = []
+    for i in range(warmup + timed):
+        pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
+        if i >= warmup:
+            kms.append(pic.get_stats()["last_move_ms"])
+    kernel = pic.last_kernel()
+    pic.close()
+    k_ms = float(np.mean(kms))
+    n_sub, n_cross = exact["n_sub"], exact["n_cross"]
+    ops = OPS_INCELL * (n_sub - n_cross) + OPS_CROSS * n_cross
+    return {"workload": f"cfg3: {cfg['n_cells']} cells, {n_p} two-stream particles, dt={dt}",
+            "precision": "fp32", "steps": timed, "warmup": warmup, "kernel": kernel,
+            "kernel_ms": k_ms, "kernel_ms_min": float(np.min(kms)), "kernel_ms_max": float(np.max(kms)),
+            "value": n_sub / (k_ms * 1e-3), "unit": UNIT,
+            "substeps_per_particle": mean, "crossing_fraction": n_cross / max(n_sub, 1),
+            "n_sub_percentile_upper_bounds": pct, "histogram_bin_width": width,
+            "roofline_frac": ops / (k_ms * 1e-3) * 1e-9 / _peak_gops(sms, "fp32", sm_max_mhz)}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -392,6 +509,9 @@ def main():
                     help="the paper's particle order (Eq. 15): consecutive particles in consecutive cells")
     ap.add_argument("--per-visit", action="store_true",
                     help="deposit per cell visit with shared fp64 atomics (P:222) instead of the end-point form")
+    ap.add_argument("--no-extra-legs", action="store_true",
+                    help="default cfg2 line only: skip the bounded configs[4] / [1] / [3] legs "
+                         "('implicit_step', 'cfg1', 'cfg3' in the JSON line)")
     ap.add_argument("--vp", action="store_true",
                     help="Vlasov-Poisson variant of the mover: orbits without the current deposit (P:281)")
     args = ap.parse_args()
@@ -540,7 +660,7 @@ def main():
 
     # ---- dominant kernel alone: CUDA events around the mover launches (library-side events)
     kms = []
-    for _ in range(min(args.steps, 5)):
+    for _ in range(min(args.steps, 20)):
         pic.move_accumulate(dEn, dEp, dt, tol, jbar_out=dj)
         kms.append(pic.get_stats()["last_move_ms"])
     k_ms = float(np.mean(kms))
@@ -618,6 +738,8 @@ def main():
                                         + NCU_TRAFFIC_SOURCE + ": all instructions by the paper's "
                                         "convention / floating-point arithmetic only",
                      "kernel": kernel_name, "kernel_ms": k_ms,
+                     "kernel_ms_launches": {"n": len(kms), "min": float(np.min(kms)),
+                                            "median": float(np.median(kms)), "max": float(np.max(kms))},
                      "ops_per_launch": ops_per_launch,
                      "peak_source": "derived: SMs x lanes x 2 x sm_max_mhz (DESIGN.md 6)",
                      "hbm_gbs_algorithmic": n_p * (24 if args.precision == "fp32" else 40) / (k_ms * 1e-3) * 1e-9},
@@ -651,6 +773,15 @@ def main():
                                      "peak": peak64, "unit": "GOp/s",
                                      "frac": ops64 / (k64 * 1e-3) * 1e-9 / peak64}}
         p64.close()
+    # ---- the other configs of BASELINE.json in the same record (bounded: ~10 s in all): the
+    # implicit step of configs[4] (fp32) and configs[1] (fp64), the mover on configs[3]
+    default_line = (args.workload == "cfg2" and args.precision == "fp32" and world == 1 and not args.n
+                    and not (args.vp or args.strided or args.per_visit or args.one_per_lane or args.no_vsort))
+    if default_line and not args.no_extra_legs:
+        del dEn, dEp, dj
+        line["implicit_step"] = extra_iaw_leg(B, torch, "cfg4", "fp32", 20, 3, args.seed, stream, sms, sm_max_mhz)
+        line["cfg1"] = extra_iaw_leg(B, torch, "cfg1", "fp64", 10, 3, args.seed, stream, sms, sm_max_mhz)
+        line["cfg3"] = extra_cfg3_leg(B, torch, args.seed, stream, sms, sm_max_mhz)
     if not args.no_cpu_baseline:
         rate, nsub_s, dts, ns = oracle_rate(cfg, args.cpu_sample)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
