@@ -35,15 +35,20 @@ UNIT = "sub-steps/s"
 # P:94-105), SURVEY 8(d) / DESIGN.md 6: per in-cell sub-step and per crossing sub-step.
 OPS_INCELL, OPS_CROSS = 43.0, 72.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one mover launch from the committed
-# `ncu --set full` capture (profiles/r1_mover_ncu.md); known only for the default workload.
+# `ncu --set full` capture (profiles/r2_mover_ncu.md; re-captured in round 3 with the same
+# result, profiles/r3_op_table.md); known only for the default workload.
 NCU_TRAFFIC_BYTES = {("cfg2", 100_000_000, "fp32"): 2.365e9, ("cfg2", 100_000_000, "fp64"): 3.970e9}
 NCU_TRAFFIC_SOURCE = "profiles/r2_mover_ncu.md (ncu --set full capture of this kernel; not measured in this run)"
 # Executed thread-operations per sub-step of the timed kernel, summed over the SASS lines of the
 # same ncu capture (source page, predicated-on thread instructions): (a) the paper's convention
 # (every instruction 1, FFMA 2, packed FFMA2 4, FMUL2 / FADD2 2), (b) floating-point arithmetic
-# only (FADD, FMUL, FFMA, their packed forms; no integer, compare, select, MUFU, memory, control).
-NCU_EXECUTED_OPS = {("cfg2", 100_000_000, "fp32", "mover2_kernel"): (46.12, 27.45),
-                    ("cfg2", 100_000_000, "fp64", "mover_kernel"): (81.22, 46.17)}
+# only (FADD, FMUL, FFMA, their packed forms; no integer, compare, select, MUFU, memory, control),
+# (c) the paper's operation classes only: FP + AL (integer, logic, compare, select,
+# min/max, conversions) + SF (MUFU), without control (BRA, BSSY, BSYNC, votes) and data movement
+# (MOV, SHFL, LDS/STS, LDG/STG, ATOMS); per-opcode table in profiles/r3_op_table.md (None: not
+# split for that kernel).
+NCU_EXECUTED_OPS = {("cfg2", 100_000_000, "fp32", "mover2_kernel"): (46.12, 27.45, 38.71),
+                    ("cfg2", 100_000_000, "fp64", "mover_kernel"): (81.22, 46.17, None)}
 
 
 def _workload(name, n, seed):
@@ -734,9 +739,13 @@ def main():
                                        if executed else None),
                      "frac_fp_only": (executed[1] * n_sub / (k_ms * 1e-3) * 1e-9 / peak_gops
                                       if executed else None),
+                     "frac_executed_paper_classes": (executed[2] * n_sub / (k_ms * 1e-3) * 1e-9 / peak_gops
+                                                     if executed and executed[2] else None),
                      "executed_source": "thread-operations per sub-step from the SASS counters of "
                                         + NCU_TRAFFIC_SOURCE + ": all instructions by the paper's "
-                                        "convention / floating-point arithmetic only",
+                                        "convention / floating-point arithmetic only / executed FP + AL + SF "
+                                        "operations without control and data movement "
+                                        "(profiles/r3_op_table.md)",
                      "kernel": kernel_name, "kernel_ms": k_ms,
                      "kernel_ms_launches": {"n": len(kms), "min": float(np.min(kms)),
                                             "median": float(np.median(kms)), "max": float(np.max(kms))},

@@ -2,8 +2,8 @@
 // particles per lane and packed FP32 arithmetic (sm_100a FFMA2 / FMUL2 / FADD2).
 //
 // Why: mover_kernel<float> is bound by instruction issue (90 % of the issue slots busy, FMA pipe
-// 47 %, profiles/r1_mover_ncu.md).  sm_100a executes fma/mul/add.f32x2 on a register pair as ONE
-// issued instruction (measured with pic_microbench, profiles/r1_microbench.md: the same FMA-pipe
+// 47 %, profiles/r2_mover_ncu.md).  sm_100a executes fma/mul/add.f32x2 on a register pair as ONE
+// issued instruction (measured with pic_microbench, profiles/r2_microbench.md: the same FMA-pipe
 // time as two scalar FFMAs with half the instructions).  The estimator (Eq. 6-8) and the
 // Crank-Nicolson update (Eq. 11) of two independent particles are the same straight-line
 // arithmetic, so each lane carries two orbits ("slots" .x and .y of float2 registers) and runs

@@ -115,7 +115,7 @@ int bin_species(pic_handle* h, SpeciesState& S, const double* dx_, const double*
 #endif
     // offset classes: 8 for the one-particle-per-lane kernels; the two-per-lane fp32 kernel
     // (64 orbits per warp) does better with 4 and twice as fine velocity classes
-    // (profiles/r1_bench.md)
+    // (profiles/r2_bench.md)
     const bool pow2 = ng > 1 && (ng & (ng - 1)) == 0;
     const bool two_per_lane = h->elem == 4 && pow2 && h->params.cn_mode == PIC_CN_DIRECT &&
         (size_t)ng * 28 <= 113 * 1024 &&
