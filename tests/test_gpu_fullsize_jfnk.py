@@ -82,6 +82,48 @@ def test_cfg2_full_size_sampled(oracle):
     assert cont <= 1e-5
     # the device rho diagnostic agrees with the oracle's
     assert G.rel_l2(pic.rho(B.PIC_STATE_NP1), rho1) < 1e-10
+    del rho0, rho1
+    # ---- jbar of the WHOLE launch against the oracle: all 1e8 orbits through the serial oracle,
+    # one call per chunk on every host core (orbits are independent given E; each call has its
+    # own raw J, summed afterwards).  Continuity fixes jbar only up to a constant and the energy
+    # identity barely constrains that constant; this pins the mean current (P-8) as well.
+    # Orbits that took another branch than the kernel's (flips, by the exact per-particle counts
+    # of the counting build) are taken out of BOTH sums: the deposit is linear in the particles,
+    # so each side's jbar of the flipped orbits alone is subtracted from its total.
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    c0h, s0h, v0h = c0.cpu().numpy(), x0.cpu().numpy() * dx, v0.cpu().numpy()
+    nsh, nch, c1h = nsub.cpu().numpy().astype(np.uint32), ncross.cpu().numpy().astype(np.uint32), c1.cpu().numpy()
+    bounds = np.linspace(0, n, 8 * cores + 1).astype(np.int64)
+    par = oracle.make_params()
+
+    def one(k):
+        a, b = int(bounds[k]), int(bounds[k + 1])
+        r = oracle.move_accumulate(ng, cfg["length"], sp["q_over_m"], sp["w_q"], c0h[a:b], s0h[a:b],
+                                   v0h[a:b], cfg["E_n"], cfg["E_np1"], dt, par)
+        flip = (r["n_sub"] != nsh[a:b]) | (r["n_cross"] != nch[a:b]) | (r["cell"] != c1h[a:b])
+        return r["J"], a + np.nonzero(flip)[0]
+
+    with ThreadPoolExecutor(max_workers=cores) as ex:
+        parts = list(ex.map(one, range(8 * cores)))
+    J_all = np.sum([q[0] for q in parts], axis=0)
+    F = np.concatenate([q[1] for q in parts])
+    print(f"[full] oracle on all {n} orbits ({cores} cores): flips={F.size}")
+    assert F.size <= 1e-3 * n
+    j_o = oracle.jbar_from_J(ng, cfg["length"], dt, J_all)
+    j_g = jbar.copy()
+    if F.size:
+        rF = oracle.move_accumulate(ng, cfg["length"], sp["q_over_m"], sp["w_q"], c0h[F], s0h[F],
+                                    v0h[F], cfg["E_n"], cfg["E_np1"], dt, par, want_state=False)
+        j_o = j_o - oracle.jbar_from_J(ng, cfg["length"], dt, rF["J"])
+        gF = G.gpu_run(cfg, "fp32", flags=B.PIC_FLAG_VSORT, subset=[F])   # same inputs, same rounding
+        j_g = j_g - gF["jbar"]
+        gF["pic"].close()
+    ej = G.rel_l2(j_g, j_o)
+    mean_err = abs(j_g.sum() - j_o.sum()) / np.abs(j_o).sum()
+    print(f"[full] jbar of the whole launch vs the oracle: rel L2 {ej:.2e}, |sum_f dj| / sum_f |j| {mean_err:.2e}")
+    assert ej <= G.TOL["fp32"]["j"] and mean_err <= 1e-6
     pic.close()
 
 
